@@ -1,0 +1,185 @@
+"""Seeded synthetic input generators (meshes and initial fields) shared by the tests, bench.py and the oracle legs.
+
+This module holds none of the method's arithmetic: it only produces node coordinates, initial conservative
+cell averages (and, for the sine case, exact derivative data) and the gas/option constants of each workload.
+The inputs stand in for the paper's workloads (section 6; BASELINE.json configs); recipe in DESIGN.md section 5.
+
+Array layouts (numpy, C order, fp64): nodes (3, nk+1, nj+1, ni+1); Q (5, nk, nj, ni); G (5, 3, nk, nj, ni);
+D (5, 12, nk, nj, ni).  Line index s = 4*axis + 2*a + b, (a, b) selecting -g/+g on the two other axes, ascending.
+"""
+import math
+
+import numpy as np
+
+GAUSS_G = 0.5 / math.sqrt(3.0)
+
+
+# ----------------------------------------------------------------------------- meshes
+def cartesian_nodes(n, lo=0.0, hi=2.0 * math.pi):
+    """Uniform periodic Cartesian mesh of n^3 (or (ni,nj,nk)) cells on [lo,hi]^3."""
+    ni, nj, nk = (n, n, n) if np.isscalar(n) else n
+    x = np.linspace(lo, hi, ni + 1); y = np.linspace(lo, hi, nj + 1); z = np.linspace(lo, hi, nk + 1)
+    Z, Y, X = np.meshgrid(z, y, x, indexing="ij")
+    return np.stack([X, Y, Z]).astype(np.float64)
+
+
+def curvilinear_nodes(n, amp=0.1):
+    """Non-orthogonal periodic mesh of BASELINE.json config 3 on [0,2pi]^3:
+    x = xi + amp sin(eta) sin(zeta), y = eta + amp sin(xi) sin(zeta), z = zeta + amp sin(xi) sin(eta)."""
+    c = cartesian_nodes(n, 0.0, 2.0 * math.pi)
+    xi, eta, zeta = c[0], c[1], c[2]
+    return np.stack([xi + amp * np.sin(eta) * np.sin(zeta),
+                     eta + amp * np.sin(xi) * np.sin(zeta),
+                     zeta + amp * np.sin(xi) * np.sin(eta)])
+
+
+def cell_centroids(nodes):
+    """Mean of the 8 nodes of each cell, shape (3, nk, nj, ni)."""
+    s = 0.0
+    for dk in (0, 1):
+        for dj in (0, 1):
+            for di in (0, 1):
+                s = s + nodes[:, dk:nodes.shape[1] - 1 + dk, dj:nodes.shape[2] - 1 + dj, di:nodes.shape[3] - 1 + di]
+    return s / 8.0
+
+
+def prim_to_cons(rho, u, v, w, p, gamma=1.4):
+    return np.stack([rho, rho * u, rho * v, rho * w, p / (gamma - 1.0) + 0.5 * rho * (u * u + v * v + w * w)])
+
+
+# ----------------------------------------------------------------------------- config 1: sine advection
+def sine_params():
+    """Accuracy test: inviscid, tau = 0."""
+    return dict(gamma=1.4, Pr=1.0, mu_ref=0.0, visc_omega=0.0, T_ref=1.0, tau_c1=0.0, tau_c2=0.0)
+
+
+def _sine_rho(s, t=0.0):
+    return 1.0 + 0.2 * np.sin(math.pi * (s - 3.0 * t))
+
+
+def sine_exact_averages(n, t=0.0):
+    """Exact cell averages of rho = 1 + 0.2 sin(pi(x+y+z-3t)) on the uniform n^3 mesh of [0,2]^3."""
+    h = 2.0 / n
+    c = (np.arange(n) + 0.5) * h
+    Z, Y, X = np.meshgrid(c, c, c, indexing="ij")
+    sinc = (math.sin(math.pi * h / 2) / (math.pi * h / 2)) ** 3
+    return 1.0 + 0.2 * sinc * np.sin(math.pi * (X + Y + Z - 3.0 * t))
+
+
+def sine_advection(n, t=0.0, gamma=1.4):
+    """State of the accuracy test at time t on the uniform n^3 mesh of [0,2]^3:
+    exact cell averages; G by the 4-point face Gauss quadrature of exact point values (Eq. 9);
+    D = exact point-value differences between paired face Gauss points (Eq. 10 without 1/|l|)."""
+    h = 2.0 / n
+    nodes = cartesian_nodes(n, 0.0, 2.0)
+    rho = sine_exact_averages(n, t)
+    c = (np.arange(n) + 0.5) * h
+    Z, Y, X = np.meshgrid(c, c, c, indexing="ij")
+    S = X + Y + Z                        # only x+y+z matters
+    g = GAUSS_G * h
+    drho_axis = np.zeros((3,) + rho.shape)       # cell-averaged d rho/dx_axis by face quadrature
+    Drho = np.zeros((12,) + rho.shape)
+    for axis in range(3):
+        k = 0
+        acc = 0.0
+        for a in (-g, g):
+            for b in (-g, g):
+                hi_ = _sine_rho(S + h / 2 + a + b, t); lo_ = _sine_rho(S - h / 2 + a + b, t)
+                Drho[4 * axis + k] = hi_ - lo_
+                acc = acc + 0.25 * (hi_ - lo_) / h
+                k += 1
+        drho_axis[axis] = acc
+    # rho U = rho, rho E = p/(gamma-1) + 1.5 rho: every variable is affine in rho
+    coef = np.array([1.0, 1.0, 1.0, 1.0, 1.5])
+    Q = prim_to_cons(rho, 1.0, 1.0, 1.0, 1.0, gamma)
+    G = coef[:, None, None, None, None] * drho_axis[None]
+    D = coef[:, None, None, None, None] * Drho[None]
+    return nodes, Q, G, D
+
+
+# ----------------------------------------------------------------------------- configs 2/3: Taylor-Green vortex
+def tgv_params(Ma=0.1, Re=1600.0, Pr=0.72):
+    """Taylor-Green vortex (BASELINE.json config 2): constant mu = 1/Re, tau = mu/p + 5 |dp|/|sum p| dt."""
+    return dict(gamma=1.4, Pr=Pr, mu_ref=1.0 / Re, visc_omega=0.0, T_ref=1.0, tau_c1=0.0, tau_c2=5.0)
+
+
+def taylor_green(nodes, Ma=0.1, gamma=1.4):
+    """Point values of the TGV initial field at the cell centroids, used as cell averages."""
+    x, y, z = cell_centroids(nodes)
+    p0 = 1.0 / (gamma * Ma * Ma)
+    u = np.sin(x) * np.cos(y) * np.cos(z)
+    v = -np.cos(x) * np.sin(y) * np.cos(z)
+    w = np.zeros_like(u)
+    p = p0 + (np.cos(2 * x) + np.cos(2 * y)) * (np.cos(2 * z) + 2.0) / 16.0
+    rho = p / p0
+    return prim_to_cons(rho, u, v, w, p, gamma)
+
+
+def free_stream(shape, gamma=1.4):
+    """Uniform state of BASELINE.json config 3: rho = 1, U = (1, 0.5, 0.25), p = 1/1.4."""
+    one = np.ones(shape)
+    return prim_to_cons(one, 1.0 * one, 0.5 * one, 0.25 * one, one / 1.4, gamma)
+
+
+# ----------------------------------------------------------------------------- configs 4/5: isotropic turbulence
+def iso_params(Ma_t, Re_lambda=72.0, k0=8.0, gamma=1.4, Pr=0.7):
+    """Decaying isotropic turbulence (BASELINE.json configs 4-5; not in the paper): power-law viscosity."""
+    p = 1.0 / (gamma * Ma_t * Ma_t)
+    uprime = 1.0 / math.sqrt(3.0); lam = 2.0 / k0
+    mu_ref = 1.0 * uprime * lam / Re_lambda
+    return dict(gamma=gamma, Pr=Pr, mu_ref=mu_ref, visc_omega=0.76, T_ref=p / 1.0, tau_c1=0.0, tau_c2=5.0)
+
+
+def iso_turbulence(n, seed, Ma_t, k0=8.0, gamma=1.4):
+    """Solenoidal random-phase velocity with E(k) ~ k^4 exp(-2 k^2/k0^2) on the periodic n^3 mesh of [0,2pi]^3,
+    rescaled to <u.u>^(1/2) = 1; rho = 1, p = 1/(gamma Ma_t^2)."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    noise = rng.standard_normal((3, n, n, n))
+    uh = np.fft.fftn(noise, axes=(1, 2, 3))
+    mag = np.abs(uh); mag[mag == 0] = 1.0
+    uh = uh / mag                                       # unit modulus, random phase, Hermitian symmetric
+    kk = np.fft.fftfreq(n, 1.0 / n)
+    KZ, KY, KX = np.meshgrid(kk, kk, kk, indexing="ij")
+    kvec = np.stack([KX, KY, KZ]); k2 = (kvec ** 2).sum(0); k2s = np.where(k2 == 0, 1.0, k2)
+    uh = uh - kvec * (kvec * uh).sum(0) / k2s           # solenoidal projection
+    kmag = np.sqrt(k2s)
+    Ek = kmag ** 4 * np.exp(-2.0 * k2 / (k0 * k0))
+    amp = np.sqrt(Ek / (2.0 * math.pi * k2s)); amp[k2 == 0] = 0.0
+    nrm = np.sqrt((np.abs(uh) ** 2).sum(0)); nrm[nrm == 0] = 1.0
+    uh = uh / nrm * amp
+    u = np.real(np.fft.ifftn(uh, axes=(1, 2, 3)))
+    u /= math.sqrt((u ** 2).sum(0).mean())
+    rho = np.ones((n, n, n)); p = np.full((n, n, n), 1.0 / (gamma * Ma_t * Ma_t))
+    # velocity array order (x, y, z) with array axes (k, j, i) = (z, y, x)
+    return prim_to_cons(rho, u[0], u[1], u[2], p, gamma)
+
+
+# ----------------------------------------------------------------------------- named workloads
+def workload(name, n=None):
+    """Returns dict(nodes, Q, G, D, params, nonlinear, cfl, steps) for the five BASELINE.json configs.
+    G, D are None when the derivative dof are bootstrapped by cgks_set_state."""
+    if name == "sine":
+        n = n or 16
+        nodes, Q, G, D = sine_advection(n)
+        return dict(nodes=nodes, Q=Q, G=G, D=D, params=sine_params(), nonlinear=1, cfl=0.5, steps=10)
+    if name == "tgv":
+        n = n or 64
+        nodes = cartesian_nodes(n)
+        return dict(nodes=nodes, Q=taylor_green(nodes), G=None, D=None, params=tgv_params(), nonlinear=1, cfl=0.5, steps=200)
+    if name == "tgv_curv":
+        n = n or 64
+        nodes = curvilinear_nodes(n)
+        return dict(nodes=nodes, Q=taylor_green(nodes), G=None, D=None, params=tgv_params(), nonlinear=1, cfl=0.5, steps=200)
+    if name == "freestream_curv":
+        n = n or 64
+        nodes = curvilinear_nodes(n)
+        return dict(nodes=nodes, Q=free_stream((n, n, n)), G=None, D=None, params=tgv_params(), nonlinear=1, cfl=0.5, steps=100)
+    if name == "iso_sub":
+        n = n or 128
+        return dict(nodes=cartesian_nodes(n), Q=iso_turbulence(n, 4, 0.5), G=None, D=None, params=iso_params(0.5),
+                    nonlinear=1, cfl=0.5, steps=500)
+    if name == "iso_sup":
+        n = n or 384
+        return dict(nodes=cartesian_nodes(n), Q=iso_turbulence(n, 5, 1.0), G=None, D=None, params=iso_params(1.0),
+                    nonlinear=1, cfl=0.5, steps=100)
+    raise KeyError(name)
