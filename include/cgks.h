@@ -1,0 +1,109 @@
+/*
+ * cgks.h -- C ABI of the B200-native CGKS-5 / S2O4 hot path (arxiv/paper_2508_08965).
+ *
+ * One S2O4 step of the fifth-order compact gas-kinetic scheme on a 3-D structured, periodic,
+ * possibly non-orthogonal mesh: compact reconstruction on the reference cell (Eq. 11-15,
+ * 17-19), GENO blend (Eq. 16), gas-kinetic flux and interface values at the face Gauss points
+ * (Eq. 1-7), update of cell averages, cell-averaged gradients and line-averaged derivatives
+ * (Eq. 8-10) and the two-stage fourth-order combine.
+ *
+ * Every step runs in hand-written fp64 CUDA kernels for sm_100a (paper_2508_08965_b200/csrc).  There is no CPU
+ * fallback: every call fails with CGKS_ECUDA when no CUDA device / kernel image is usable.
+ *
+ * Conventions
+ *  - All array arguments named d_* are DEVICE pointers owned by the caller, fp64, structure-of-arrays, i fastest:
+ *      nodes [3][nk+1][nj+1][ni+1]   node coordinates (x, y, z planes)
+ *      Q     [5][nk][nj][ni]         cell averages of (rho, rho U, rho V, rho W, rho E)
+ *      G     [5][3][nk][nj][ni]      cell-averaged PHYSICAL gradients, index 3*v + dir         (Eq. 9)
+ *      D     [5][12][nk][nj][ni]     line DIFFERENCES Q(x_G2) - Q(x_G1) (Eq. 10 times |l_G|, Eq. 19 row 4),
+ *                                    index 12*v + s, s = 4*axis + 2*a + b, (a,b) in {0,1}^2 selecting -g/+g
+ *                                    (g = 1/(2 sqrt 3)) along the two other axes in ascending axis order
+ *  - Other pointers (params, dt_host, bytes, out) are HOST pointers.
+ *  - The mesh is periodic in all three index directions; node planes 0 and n of each direction
+ *    must differ by a constant vector (checked by cgks_create).
+ *  - The library never allocates device memory: the caller passes one workspace (cgks_workspace_bytes) and keeps
+ *    it alive until cgks_destroy.  The context itself (host memory) is owned by the library.
+ *  - Calls enqueue work on the stream given to cgks_create and return without waiting, except cgks_create
+ *    (validates the mesh), cgks_compute_dt (returns a host double) and cgks_status, which synchronise the stream.
+ *  - Return value: 0 on success, negative error code otherwise; cgks_last_error gives a message.
+ */
+#ifndef CGKS_H
+#define CGKS_H
+#include <stddef.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct cgks_ctx cgks_ctx;
+
+enum {
+  CGKS_OK = 0,
+  CGKS_EINVAL = -1,        /* bad argument, ni/nj/nk < 4, non-periodic node array, det J0 <= 0 or volume <= 0 */
+  CGKS_ENOMEM = -2,        /* workspace too small                                                              */
+  CGKS_ECUDA = -3,         /* CUDA runtime error (including "no device")                                       */
+  CGKS_ENONPHYSICAL = -4   /* a cell average with rho <= 0 or p <= 0 appeared after a stage                    */
+};
+
+typedef struct {
+  double gamma, Pr, mu_ref;   /* mu_ref = 0 -> inviscid                                                        */
+  double visc_omega, T_ref;   /* mu = mu_ref (T/T_ref)^omega, T = p/rho; omega = 0 -> constant                */
+  double tau_c1, tau_c2;      /* tau = mu/p + c1 dt + c2 |pl-pr|/|pl+pr| dt: inviscid 0.05, 5;
+                                 viscous 0, 5; accuracy test 0, 0 (tau = 0)                      */
+  int    nonlinear;           /* 1 = GENO blend, 0 = linear reconstruction (chi = 1)            */
+  double geno_C, geno_eps;    /* tanh constant C = 5 (reading G3), epsilon = 1e-15    */
+  int    geno_r;              /* r = 2; only r = 2 is implemented                               */
+} cgks_params;
+
+/* Bytes of device workspace for a mesh of ni x nj x nk cells (state, stage buffers, metrics, and the slab buffers
+   of reconstructed face values and face fluxes).  `budget_bytes` = 0 asks for the default (largest useful slab up
+   to ~48 GB of slab buffers); otherwise the slab depth is reduced so that the total stays below the budget. */
+int cgks_workspace_bytes(int ni, int nj, int nk, size_t budget_bytes, size_t* bytes);
+
+/* Builds the mesh metrics (J0 of Eq. 18, cell volumes by the Appendix quadrature, face vector areas, DESIGN.md
+   readings R1-R2) and the context.  d_nodes is read during the call only. */
+int cgks_create(cgks_ctx** out, int ni, int nj, int nk, const double* d_nodes, const cgks_params* params,
+                void* d_workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* Copies the state in.  d_G and/or d_D may be NULL: the missing derivative dof are bootstrapped from Q by
+   fourth-order central differences in index space (reading S2). */
+int cgks_set_state(cgks_ctx*, const double* d_Q, const double* d_G, const double* d_D);
+
+/* Copies the state out (any pointer may be NULL). */
+int cgks_get_state(cgks_ctx*, double* d_Q, double* d_G, double* d_D);
+
+/* dt = cfl / max_cells sum_d (|U.n_d| + c)/h_d, capped by cfl h^2/(3 nu) for viscous flow (PAPER.md:342,
+   DESIGN.md reading S3).  Synchronises; returns CGKS_ENONPHYSICAL if an earlier stage flagged a bad cell. */
+int cgks_compute_dt(cgks_ctx*, double cfl, double* dt_host);
+
+/* One two-stage fourth-order step of size dt.  Asynchronous. */
+int cgks_step(cgks_ctx*, double dt);
+
+/* Synchronises and returns CGKS_OK, CGKS_ECUDA or CGKS_ENONPHYSICAL for the work enqueued so far. */
+int cgks_status(cgks_ctx*);
+
+/* Same as cgks_set_state / cgks_step / cgks_get_state but with HOST buffers: copies the state host->device, runs
+   `nsteps` steps with dt from the CFL condition each step, copies the state back (used for end-to-end timing). */
+int cgks_run_host(cgks_ctx*, const double* h_Q, const double* h_G, const double* h_D, double cfl, int nsteps,
+                  double* h_Q_out, double* h_G_out, double* h_D_out);
+
+/* Number of kernels launched by the library on this context so far (for bench.py's gpu_launches). */
+long cgks_launch_count(const cgks_ctx*);
+
+/* Device-side duration in milliseconds of the kernels of one class accumulated by the last cgks_step when profiling
+   is switched on with cgks_set_profiling(ctx, 1): 0 reconstruction, 1 flux, 2 update, 3 cfl.  Profiling inserts
+   CUDA events on the stream and synchronises at the end of the step. */
+int cgks_set_profiling(cgks_ctx*, int on);
+int cgks_kernel_ms(const cgks_ctx*, int which, double* ms, long* launches);
+
+/* Debug/testing taps (device pointers, valid until the next cgks_step): reconstructed face values of slab-resident
+   cells are not exposed; instead this returns chi of the last reconstruction, [5][nk][nj][ni], copied to d_chi. */
+int cgks_get_chi(cgks_ctx*, double* d_chi);
+
+int cgks_destroy(cgks_ctx*);
+const char* cgks_last_error(const cgks_ctx*);
+const char* cgks_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,172 @@
+"""Thin Python binding of the C ABI in include/cgks.h (argument marshalling only).
+
+PyTorch is used for device memory and streams; every step of the path runs in the CUDA kernels of libcgks.so.
+There is no CPU fallback: a missing library or device raises."""
+import ctypes as C
+import os
+
+import numpy as np
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libcgks.so")
+
+CGKS_OK, CGKS_EINVAL, CGKS_ENOMEM, CGKS_ECUDA, CGKS_ENONPHYSICAL = 0, -1, -2, -3, -4
+KERNEL_CLASSES = {"recon": 0, "flux": 1, "update": 2, "cfl": 3, "other": 4}
+
+
+class cgks_params(C.Structure):
+    _fields_ = [("gamma", C.c_double), ("Pr", C.c_double), ("mu_ref", C.c_double),
+                ("visc_omega", C.c_double), ("T_ref", C.c_double),
+                ("tau_c1", C.c_double), ("tau_c2", C.c_double),
+                ("nonlinear", C.c_int), ("geno_C", C.c_double), ("geno_eps", C.c_double),
+                ("geno_r", C.c_int)]
+
+
+class CgksError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__("cgks error %d: %s" % (code, msg))
+        self.code = code
+
+
+_lib = None
+_vp = C.c_void_p
+
+
+def lib():
+    """Loads libcgks.so; raises if it has not been built (python -m paper_2508_08965_b200.build)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError("CUDA extension %s is missing: run `python paper_2508_08965_b200/build.py`" % LIB_PATH)
+        L = C.CDLL(LIB_PATH)
+        L.cgks_workspace_bytes.argtypes = [C.c_int, C.c_int, C.c_int, C.c_size_t, C.POINTER(C.c_size_t)]
+        L.cgks_create.argtypes = [C.POINTER(_vp), C.c_int, C.c_int, C.c_int, _vp, C.POINTER(cgks_params), _vp, C.c_size_t, _vp]
+        L.cgks_set_state.argtypes = [_vp, _vp, _vp, _vp]
+        L.cgks_get_state.argtypes = [_vp, _vp, _vp, _vp]
+        L.cgks_compute_dt.argtypes = [_vp, C.c_double, C.POINTER(C.c_double)]
+        L.cgks_step.argtypes = [_vp, C.c_double]
+        L.cgks_status.argtypes = [_vp]
+        L.cgks_run_host.argtypes = [_vp, _vp, _vp, _vp, C.c_double, C.c_int, _vp, _vp, _vp]
+        L.cgks_launch_count.argtypes = [_vp]; L.cgks_launch_count.restype = C.c_long
+        L.cgks_set_profiling.argtypes = [_vp, C.c_int]
+        L.cgks_kernel_ms.argtypes = [_vp, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_long)]
+        L.cgks_get_chi.argtypes = [_vp, _vp]
+        L.cgks_destroy.argtypes = [_vp]
+        L.cgks_last_error.argtypes = [_vp]; L.cgks_last_error.restype = C.c_char_p
+        L.cgks_version.restype = C.c_char_p
+        _lib = L
+    return _lib
+
+
+def make_params(gamma=1.4, Pr=1.0, mu_ref=0.0, visc_omega=0.0, T_ref=1.0, tau_c1=0.0, tau_c2=0.0,
+                nonlinear=1, geno_C=5.0, geno_eps=1e-15, geno_r=2):
+    return cgks_params(gamma, Pr, mu_ref, visc_omega, T_ref, tau_c1, tau_c2, int(nonlinear), geno_C, geno_eps, int(geno_r))
+
+
+def workspace_bytes(ni, nj, nk, budget_bytes=0):
+    out = C.c_size_t(0)
+    rc = lib().cgks_workspace_bytes(ni, nj, nk, budget_bytes, C.byref(out))
+    if rc:
+        raise CgksError(rc, "cgks_workspace_bytes")
+    return out.value
+
+
+def _dev(a, device):
+    if a is None:
+        return None
+    if isinstance(a, np.ndarray):
+        a = torch.from_numpy(np.ascontiguousarray(a, dtype=np.float64))
+    return a.to(device=device, dtype=torch.float64).contiguous()
+
+
+def _ptr(t):
+    return None if t is None else _vp(t.data_ptr())
+
+
+class Solver:
+    """cgks_create / cgks_set_state / cgks_compute_dt / cgks_step / cgks_get_state on one CUDA device.
+
+    nodes (3, nk+1, nj+1, ni+1); Q (5, nk, nj, ni); G (5, 3, nk, nj, ni); D (5, 12, nk, nj, ni)."""
+
+    def __init__(self, nodes, params, device="cuda:0", budget_bytes=0):
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2508_08965_b200 needs a CUDA device (no CPU fallback)")
+        self.device = torch.device(device)
+        self._h = _vp(None)
+        L = lib()
+        nodes = _dev(nodes, self.device)
+        self.nk, self.nj, self.ni = (int(s) - 1 for s in nodes.shape[1:])
+        self.n = self.ni * self.nj * self.nk
+        self.params = params if isinstance(params, cgks_params) else make_params(**params)
+        nbytes = workspace_bytes(self.ni, self.nj, self.nk, budget_bytes)
+        with torch.cuda.device(self.device):
+            self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+            self.stream = torch.cuda.current_stream(self.device)
+            rc = L.cgks_create(C.byref(self._h), self.ni, self.nj, self.nk, _ptr(nodes), C.byref(self.params),
+                               _vp(self.workspace.data_ptr()), nbytes, _vp(self.stream.cuda_stream))
+        if rc:
+            self._h = _vp(None)
+            raise CgksError(rc, "cgks_create failed (see stderr)")
+
+    def _check(self, rc):
+        if rc:
+            raise CgksError(rc, lib().cgks_last_error(self._h).decode())
+
+    def close(self):
+        if self._h:
+            lib().cgks_destroy(self._h); self._h = _vp(None)
+        self.workspace = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def set_state(self, Q, G=None, D=None):
+        Q, G, D = _dev(Q, self.device), _dev(G, self.device), _dev(D, self.device)
+        assert Q.numel() == 5 * self.n
+        self._check(lib().cgks_set_state(self._h, _ptr(Q), _ptr(G), _ptr(D)))
+        torch.cuda.current_stream(self.device).synchronize()      # the inputs may be temporaries
+
+    def get_state(self):
+        s = (self.nk, self.nj, self.ni)
+        Q = torch.empty((5,) + s, dtype=torch.float64, device=self.device)
+        G = torch.empty((5, 3) + s, dtype=torch.float64, device=self.device)
+        D = torch.empty((5, 12) + s, dtype=torch.float64, device=self.device)
+        self._check(lib().cgks_get_state(self._h, _ptr(Q), _ptr(G), _ptr(D)))
+        return Q, G, D
+
+    def compute_dt(self, cfl):
+        out = C.c_double(0.0)
+        self._check(lib().cgks_compute_dt(self._h, float(cfl), C.byref(out)))
+        return out.value
+
+    def step(self, dt):
+        self._check(lib().cgks_step(self._h, float(dt)))
+
+    def status(self):
+        self._check(lib().cgks_status(self._h))
+
+    def chi(self):
+        out = torch.empty((5, self.nk, self.nj, self.ni), dtype=torch.float64, device=self.device)
+        self._check(lib().cgks_get_chi(self._h, _ptr(out)))
+        return out
+
+    def run_host(self, Q, G, D, cfl, nsteps, out_Q, out_G=None, out_D=None):
+        """Host (ideally pinned) tensors in and out; H2D + nsteps steps + D2H inside the call."""
+        def hp(t):
+            return None if t is None else _vp(t.data_ptr())
+        self._check(lib().cgks_run_host(self._h, hp(Q), hp(G), hp(D), float(cfl), int(nsteps), hp(out_Q), hp(out_G), hp(out_D)))
+
+    def launch_count(self):
+        return int(lib().cgks_launch_count(self._h))
+
+    def set_profiling(self, on):
+        self._check(lib().cgks_set_profiling(self._h, int(on)))
+
+    def kernel_ms(self, which):
+        ms = C.c_double(0.0); nl = C.c_long(0)
+        self._check(lib().cgks_kernel_ms(self._h, KERNEL_CLASSES[which], C.byref(ms), C.byref(nl)))
+        return ms.value, nl.value

@@ -1,0 +1,38 @@
+"""Builds paper_2508_08965_b200/libcgks.so (hand-written CUDA for sm_100a) in-tree with nvcc."""
+import os
+import subprocess
+import sys
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+CSRC = os.path.join(HERE, "csrc")
+LIB = os.path.join(HERE, "libcgks.so")
+SOURCES = ["cgks_api.cu"]
+HEADERS = ["cgks_common.cuh", "kernels_setup.cuh", "kernels_stage.cuh", "gks_flux.cuh", "recon_gen.cuh"]
+NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
+              "-Xcompiler", "-fPIC", "-shared"]
+
+
+def _newer(a, b):
+    return os.path.getmtime(a) > os.path.getmtime(b)
+
+
+def generate(force=False):
+    gen = os.path.join(CSRC, "gen_recon.py"); out = os.path.join(CSRC, "recon_gen.cuh")
+    if force or not os.path.exists(out) or _newer(gen, out):
+        subprocess.check_call([sys.executable, gen])
+    return out
+
+
+def build(force=False, verbose=False):
+    generate(force)
+    deps = [os.path.join(CSRC, f) for f in SOURCES + HEADERS] + [os.path.join(HERE, "..", "include", "cgks.h")]
+    if not force and os.path.exists(LIB) and all(not _newer(d, LIB) for d in deps):
+        return LIB
+    nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES]
+    subprocess.check_call(cmd)
+    return LIB
+
+
+if __name__ == "__main__":
+    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))

@@ -1,0 +1,353 @@
+// cgks_api.cu -- C ABI (include/cgks.h) of the CGKS-5 / S2O4 hot path: workspace carving, slab pipeline, launches.
+#include "../../include/cgks.h"
+#include "cgks_common.cuh"
+#include "kernels_setup.cuh"
+#include "kernels_stage.cuh"
+
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+#include <string>
+#include <vector>
+
+using namespace cgks;
+
+namespace {
+constexpr int TPB = 128;
+constexpr size_t ALIGN = 256;
+constexpr size_t DEFAULT_SLAB_BYTES = (size_t)48 << 30;
+
+enum { KC_RECON = 0, KC_FLUX = 1, KC_UPDATE = 2, KC_CFL = 3, KC_OTHER = 4, KC_N = 5 };
+
+struct EvRec { int cls; cudaEvent_t a, b; };
+
+size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
+size_t state_bytes(long n) { return align_up((size_t)NSTATE * n * 8); }
+size_t slot_bytes(long plane) { return (size_t)(NPV + NFX) * plane * 8; }
+}  // namespace
+
+struct cgks_ctx {
+  Mesh mesh{};
+  cgks_params prm{};
+  cudaStream_t stream = nullptr;
+  double* W[3] = { nullptr, nullptr, nullptr };
+  int cur = 0, star = 1, save = 2;
+  double* met = nullptr;
+  double* chi = nullptr;
+  double* pv = nullptr;
+  double* fx = nullptr;
+  unsigned long long* d_dt = nullptr;   // [1] bit pattern of the reduced dt
+  int* d_flags = nullptr;               // [0..2] geometry, [3] non-physical state
+  int S = 0;                            // slab depth in k-planes; S == nk: whole mesh resident
+  int slots_pv = 0, slots_fx = 0;
+  long launches = 0;
+  int profiling = 0;
+  std::vector<EvRec> events;
+  std::vector<cudaEvent_t> pool;
+  double ms[KC_N] = { 0, 0, 0, 0, 0 };
+  long nl[KC_N] = { 0, 0, 0, 0, 0 };
+  std::string err;
+};
+
+static int fail(cgks_ctx* c, int code, const char* msg) { if (c) c->err = msg; return code; }
+static int cuda_fail(cgks_ctx* c, cudaError_t e, const char* where) {
+  if (c) c->err = std::string(where) + ": " + cudaGetErrorString(e);
+  return CGKS_ECUDA;
+}
+#define CK(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail(c, e_, #call); } while (0)
+
+extern "C" const char* cgks_version(void) { return "cgks-b200 0.1 (sm_100a, fp64)"; }
+extern "C" const char* cgks_last_error(const cgks_ctx* c) { return c ? c->err.c_str() : "null context"; }
+extern "C" long cgks_launch_count(const cgks_ctx* c) { return c ? c->launches : 0; }
+
+static size_t fixed_bytes(long n, bool with_metrics) {
+  size_t b = 3 * state_bytes(n) + align_up((size_t)5 * n * 8) + align_up(64);
+  if (with_metrics) b += align_up((size_t)NMET * n * 8);
+  return b;
+}
+
+extern "C" int cgks_workspace_bytes(int ni, int nj, int nk, size_t budget, size_t* bytes) {
+  if (ni < 4 || nj < 4 || nk < 4 || !bytes) return CGKS_EINVAL;
+  const long plane = (long)ni * nj, n = plane * nk;
+  const size_t fixed = fixed_bytes(n, true);
+  const size_t full = (size_t)nk * slot_bytes(plane);           // whole mesh resident
+  size_t slab = full;
+  const size_t cap = budget ? (budget > fixed ? budget - fixed : 0) : DEFAULT_SLAB_BYTES;
+  if (slab > cap) {
+    long S = (long)(cap / slot_bytes(plane)) - 2;
+    if (S < 2) S = 2;
+    slab = (size_t)(S + 2) * slot_bytes(plane);
+  }
+  *bytes = fixed + align_up(slab) + ALIGN;
+  return CGKS_OK;
+}
+
+// ---- launch helpers ---------------------------------------------------------------------------------------------
+static cudaEvent_t get_event(cgks_ctx* c) {
+  if (!c->pool.empty()) { cudaEvent_t e = c->pool.back(); c->pool.pop_back(); return e; }
+  cudaEvent_t e; cudaEventCreate(&e); return e;
+}
+struct Timed {
+  cgks_ctx* c; int cls; cudaEvent_t a = nullptr, b = nullptr;
+  Timed(cgks_ctx* c_, int cls_) : c(c_), cls(cls_) {
+    c->launches++;
+    if (c->profiling) { a = get_event(c); b = get_event(c); cudaEventRecord(a, c->stream); }
+  }
+  ~Timed() { if (c->profiling) { cudaEventRecord(b, c->stream); c->events.push_back({ cls, a, b }); } }
+};
+static void collect_events(cgks_ctx* c) {
+  for (auto& e : c->events) {
+    float ms = 0; cudaEventElapsedTime(&ms, e.a, e.b);
+    c->ms[e.cls] += ms; c->nl[e.cls]++;
+    c->pool.push_back(e.a); c->pool.push_back(e.b);
+  }
+  c->events.clear();
+}
+
+static GasConst gas_const(const cgks_params& p) {
+  GasConst g;
+  g.K = (5.0 - 3.0 * p.gamma) / (p.gamma - 1.0);
+  g.Pr_fix = (p.mu_ref > 0.0 && p.Pr != 1.0) ? (1.0 / p.Pr - 1.0) : 0.0;
+  g.mu_ref = p.mu_ref; g.omega = p.visc_omega; g.T_ref = p.T_ref; g.c1 = p.tau_c1; g.c2 = p.tau_c2;
+  return g;
+}
+
+// ---- create / destroy -------------------------------------------------------------------------------------------
+extern "C" int cgks_create(cgks_ctx** out, int ni, int nj, int nk, const double* d_nodes, const cgks_params* params,
+                           void* ws, size_t ws_bytes, void* stream) {
+  if (!out) return CGKS_EINVAL;
+  *out = nullptr;
+  if (ni < 4 || nj < 4 || nk < 4 || !d_nodes || !params || !ws) return CGKS_EINVAL;
+  if (params->geno_r != 2 || !(params->gamma > 1.0) || !(params->gamma < 5.0 / 3.0 + 1e-12)) return CGKS_EINVAL;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return CGKS_ECUDA;
+  cgks_ctx* c = new cgks_ctx();
+  c->prm = *params; c->stream = (cudaStream_t)stream;
+  Mesh& m = c->mesh;
+  m.ni = ni; m.nj = nj; m.nk = nk; m.plane = (long)ni * nj; m.n = m.plane * nk; m.cart = 0; m.met = nullptr;
+  const long n = m.n;
+  // carve the workspace: [flags+dt][state x3][chi][metrics (general meshes only)][slab buffers]
+  char* base = (char*)(((uintptr_t)ws + ALIGN - 1) / ALIGN * ALIGN);
+  char* end = (char*)ws + ws_bytes;
+  char* p = base;
+  if (p + fixed_bytes(n, false) > end) { delete c; return CGKS_ENOMEM; }
+  c->d_flags = (int*)p; c->d_dt = (unsigned long long*)(p + 32); p += align_up(64);
+  for (int b = 0; b < 3; b++) { c->W[b] = (double*)p; p += state_bytes(n); }
+  c->chi = (double*)p; p += align_up((size_t)5 * n * 8);
+  int rc = CGKS_OK;
+  auto bail = [&](int code, const char* msg) { c->err = msg; rc = code; };
+  do {
+    if (cudaMemsetAsync(c->d_flags, 0, 64, c->stream) != cudaSuccess) { bail(CGKS_ECUDA, "cudaMemsetAsync failed"); break; }
+    const unsigned gridg = (unsigned)((n + TPB - 1) / TPB);
+    // pass 1: validity + uniform-Cartesian detection (no metric storage)
+    geometry_kernel<<<gridg, TPB, 0, c->stream>>>(ni, nj, nk, d_nodes, nullptr, c->d_flags); c->launches++;
+    int flags[4] = { 0, 0, 0, 0 };
+    cudaError_t e = cudaMemcpyAsync(flags, c->d_flags, sizeof flags, cudaMemcpyDeviceToHost, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    if (e != cudaSuccess) { c->err = std::string("geometry pass: ") + cudaGetErrorString(e); rc = CGKS_ECUDA; break; }
+    if (flags[1]) { bail(CGKS_EINVAL, "mesh has a cell with det J0 <= 0 or volume <= 0"); break; }
+    if (flags[2]) { bail(CGKS_EINVAL, "node array is not periodic"); break; }
+    m.cart = flags[0] ? 0 : 1;
+    if (m.cart) {
+      // h = period / n from four corner nodes
+      const long ns = (long)(ni + 1) * (nj + 1) * (nk + 1);
+      auto node = [&](int comp, int i, int j, int k, double* v) {
+        return cudaMemcpy(v, d_nodes + comp * ns + ((long)k * (nj + 1) + j) * (ni + 1) + i, 8, cudaMemcpyDeviceToHost);
+      };
+      double o[3], a;
+      for (int r = 0; r < 3; r++) node(r, 0, 0, 0, &o[r]);
+      node(0, ni, 0, 0, &a); m.h[0] = (a - o[0]) / ni;
+      node(1, 0, nj, 0, &a); m.h[1] = (a - o[1]) / nj;
+      node(2, 0, 0, nk, &a); m.h[2] = (a - o[2]) / nk;
+    } else {
+      if (p + align_up((size_t)NMET * n * 8) > end) { bail(CGKS_ENOMEM, "workspace too small for the mesh metrics"); break; }
+      c->met = (double*)p; p += align_up((size_t)NMET * n * 8);
+      m.met = c->met;
+      geometry_kernel<<<gridg, TPB, 0, c->stream>>>(ni, nj, nk, d_nodes, c->met, c->d_flags); c->launches++;
+      e = cudaStreamSynchronize(c->stream);
+      if (e != cudaSuccess) { c->err = std::string("geometry pass 2: ") + cudaGetErrorString(e); rc = CGKS_ECUDA; break; }
+    }
+    // slab buffers from what is left
+    const size_t left = (size_t)(end - p);
+    const size_t sb = slot_bytes(m.plane);
+    long slots = (long)(left / sb);
+    if (slots >= nk) { c->S = nk; c->slots_pv = nk; c->slots_fx = nk; }
+    else {
+      // S+2 pv slots and S+1 fx slots; fx slots are smaller, so (S+2) full slots always suffice
+      long S = slots - 2;
+      if (S < 2) { bail(CGKS_ENOMEM, "workspace too small for a slab of two k-planes"); break; }
+      if (S > nk) S = nk;
+      c->S = (int)S; c->slots_pv = (int)S + 2; c->slots_fx = (int)S + 1;
+    }
+    c->pv = (double*)p; p += (size_t)NPV * c->slots_pv * m.plane * 8;
+    c->fx = (double*)p;
+    cudaMemsetAsync(c->d_flags, 0, 64, c->stream);
+  } while (0);
+  if (rc != CGKS_OK) {
+    // keep the context alive only long enough to report: the caller gets the message through a static buffer
+    static std::string last; last = c->err; delete c;
+    fprintf(stderr, "cgks_create: %s\n", last.c_str());
+    return rc;
+  }
+  *out = c;
+  return CGKS_OK;
+}
+
+extern "C" int cgks_destroy(cgks_ctx* c) {
+  if (!c) return CGKS_EINVAL;
+  cudaStreamSynchronize(c->stream);
+  for (auto& e : c->events) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
+  for (auto& e : c->pool) cudaEventDestroy(e);
+  delete c;
+  return CGKS_OK;
+}
+
+// ---- state ------------------------------------------------------------------------------------------------------
+extern "C" int cgks_set_state(cgks_ctx* c, const double* Q, const double* G, const double* D) {
+  if (!c || !Q) return CGKS_EINVAL;
+  const Mesh& m = c->mesh;
+  dim3 grid((unsigned)((m.n + TPB - 1) / TPB), 5);
+  { Timed t(c, KC_OTHER); set_state_kernel<<<grid, TPB, 0, c->stream>>>(m, Q, G, D, c->W[c->cur]); }
+  CK(cudaMemsetAsync(c->d_flags + 3, 0, sizeof(int), c->stream));
+  CK(cudaGetLastError());
+  return CGKS_OK;
+}
+
+extern "C" int cgks_get_state(cgks_ctx* c, double* Q, double* G, double* D) {
+  if (!c) return CGKS_EINVAL;
+  const Mesh& m = c->mesh;
+  dim3 grid((unsigned)((m.n + TPB - 1) / TPB), 5);
+  { Timed t(c, KC_OTHER); get_state_kernel<<<grid, TPB, 0, c->stream>>>(m, c->W[c->cur], Q, G, D); }
+  CK(cudaGetLastError());
+  return CGKS_OK;
+}
+
+extern "C" int cgks_get_chi(cgks_ctx* c, double* d_chi) {
+  if (!c || !d_chi) return CGKS_EINVAL;
+  CK(cudaMemcpyAsync(d_chi, c->chi, (size_t)5 * c->mesh.n * 8, cudaMemcpyDeviceToDevice, c->stream));
+  return CGKS_OK;
+}
+
+extern "C" int cgks_status(cgks_ctx* c) {
+  if (!c) return CGKS_EINVAL;
+  int flag = 0;
+  CK(cudaMemcpyAsync(&flag, c->d_flags + 3, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+  CK(cudaStreamSynchronize(c->stream));
+  CK(cudaGetLastError());
+  if (flag) return fail(c, CGKS_ENONPHYSICAL, "a cell average with rho <= 0 or p <= 0 appeared");
+  return CGKS_OK;
+}
+
+// ---- time step ---------------------------------------------------------------------------------------------------
+extern "C" int cgks_compute_dt(cgks_ctx* c, double cfl, double* dt_host) {
+  if (!c || !dt_host || !(cfl > 0.0)) return CGKS_EINVAL;
+  const Mesh& m = c->mesh;
+  const unsigned long long inf_bits = 0x7FF0000000000000ull;
+  CK(cudaMemcpyAsync(c->d_dt, &inf_bits, 8, cudaMemcpyHostToDevice, c->stream));
+  CflPrm p{ c->prm.gamma, c->prm.mu_ref, c->prm.visc_omega, c->prm.T_ref, cfl };
+  long blocks = (m.n + 255) / 256; if (blocks > 148 * 16) blocks = 148 * 16;
+  { Timed t(c, KC_CFL); cfl_kernel<<<(unsigned)blocks, 256, 0, c->stream>>>(m, c->W[c->cur], p, c->d_dt, c->d_flags + 3); }
+  unsigned long long bits = 0; int flag = 0;
+  CK(cudaMemcpyAsync(&bits, c->d_dt, 8, cudaMemcpyDeviceToHost, c->stream));
+  CK(cudaMemcpyAsync(&flag, c->d_flags + 3, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+  CK(cudaStreamSynchronize(c->stream));
+  CK(cudaGetLastError());
+  if (flag) return fail(c, CGKS_ENONPHYSICAL, "a cell average with rho <= 0 or p <= 0 appeared");
+  memcpy(dt_host, &bits, 8);
+  return CGKS_OK;
+}
+
+// ---- one S2O4 step -------------------------------------------------------------------------------------------------
+template <bool CART>
+static void launch_flux(cgks_ctx* c, const Slab& sl, const double* Win, double dt, int kA, int cnt, int stage) {
+  const Mesh& m = c->mesh;
+  const long nt = (long)cnt * m.plane;
+  dim3 grid((unsigned)((nt + TPB - 1) / TPB), 4);
+  const GasConst gc = gas_const(c->prm);
+  { Timed t(c, KC_FLUX); flux_kernel<CART, 0><<<grid, TPB, 0, c->stream>>>(m, sl, Win, c->pv, c->fx, gc, dt, kA, nt, stage); }
+  { Timed t(c, KC_FLUX); flux_kernel<CART, 1><<<grid, TPB, 0, c->stream>>>(m, sl, Win, c->pv, c->fx, gc, dt, kA, nt, stage); }
+  { Timed t(c, KC_FLUX); flux_kernel<CART, 2><<<grid, TPB, 0, c->stream>>>(m, sl, Win, c->pv, c->fx, gc, dt, kA, nt, stage); }
+}
+
+template <bool CART>
+static void run_stage(cgks_ctx* c, int stage, double dt) {
+  const Mesh& m = c->mesh;
+  const double* Win = (stage == 1) ? c->W[c->cur] : c->W[c->star];
+  ReconPrm rp{ c->prm.nonlinear, c->prm.geno_C, c->prm.geno_eps, 1.0 / tanh(c->prm.geno_C), c->prm.gamma };
+  Slab sl; sl.slots_pv = c->slots_pv; sl.slots_fx = c->slots_fx;
+  sl.stride_pv = (long)c->slots_pv * m.plane; sl.stride_fx = (long)c->slots_fx * m.plane;
+  auto recon = [&](int kA, int cnt) {
+    const long nt = (long)cnt * m.plane;
+    dim3 grid((unsigned)((nt + TPB - 1) / TPB), 5);
+    Timed t(c, KC_RECON);
+    recon_kernel<CART><<<grid, TPB, 0, c->stream>>>(m, sl, Win, c->pv, c->chi, rp, kA, nt, c->d_flags + 3);
+  };
+  auto update = [&](int kA, int cnt) {
+    const long nt = (long)cnt * m.plane;
+    dim3 grid((unsigned)((nt + TPB - 1) / TPB), 5);
+    Timed t(c, KC_UPDATE);
+    update_kernel<CART><<<grid, TPB, 0, c->stream>>>(m, sl, c->fx, c->W[c->cur], c->W[c->star], c->W[c->save], dt, kA, nt, stage);
+  };
+  if (c->S >= m.nk) {                       // whole mesh resident: no recomputation
+    sl.kbase = 0;
+    recon(0, m.nk); launch_flux<CART>(c, sl, Win, dt, 0, m.nk, stage); update(0, m.nk);
+    return;
+  }
+  for (int k0 = 0; k0 < m.nk; k0 += c->S) {
+    const int k1 = (k0 + c->S < m.nk) ? k0 + c->S : m.nk;
+    sl.kbase = (k0 == 0) ? m.nk - 1 : k0 - 1;
+    recon(sl.kbase, k1 - k0 + 2);                                   // planes k0-1 .. k1
+    launch_flux<CART>(c, sl, Win, dt, sl.kbase, k1 - k0 + 1, stage); // cells of planes k0-1 .. k1-1 own the needed faces
+    update(k0, k1 - k0);
+  }
+}
+
+extern "C" int cgks_step(cgks_ctx* c, double dt) {
+  if (!c || !(dt > 0.0)) return CGKS_EINVAL;
+  for (int stage = 1; stage <= 2; stage++) {
+    if (c->mesh.cart) run_stage<true>(c, stage, dt); else run_stage<false>(c, stage, dt);
+  }
+  CK(cudaGetLastError());
+  // the saved buffer now holds the state at t_n+1
+  const int old = c->cur; c->cur = c->save; c->save = old;
+  if (c->profiling) { CK(cudaStreamSynchronize(c->stream)); collect_events(c); }
+  return CGKS_OK;
+}
+
+extern "C" int cgks_set_profiling(cgks_ctx* c, int on) {
+  if (!c) return CGKS_EINVAL;
+  c->profiling = on ? 1 : 0;
+  for (int i = 0; i < KC_N; i++) { c->ms[i] = 0; c->nl[i] = 0; }
+  return CGKS_OK;
+}
+
+extern "C" int cgks_kernel_ms(const cgks_ctx* c, int which, double* ms, long* launches) {
+  if (!c || which < 0 || which >= KC_N) return CGKS_EINVAL;
+  if (ms) *ms = c->ms[which];
+  if (launches) *launches = c->nl[which];
+  return CGKS_OK;
+}
+
+// ---- end-to-end with host buffers ------------------------------------------------------------------------------------
+extern "C" int cgks_run_host(cgks_ctx* c, const double* hQ, const double* hG, const double* hD, double cfl, int nsteps,
+                             double* oQ, double* oG, double* oD) {
+  if (!c || !hQ || nsteps < 0) return CGKS_EINVAL;
+  const Mesh& m = c->mesh; const long n = m.n;
+  // stage the host arrays through the (currently unused) stage buffer, then run the ordinary set_state path
+  double* tmp = c->W[c->star];
+  CK(cudaMemcpyAsync(tmp, hQ, (size_t)5 * n * 8, cudaMemcpyHostToDevice, c->stream));
+  if (hG) CK(cudaMemcpyAsync(tmp + 5 * n, hG, (size_t)15 * n * 8, cudaMemcpyHostToDevice, c->stream));
+  if (hD) CK(cudaMemcpyAsync(tmp + 20 * n, hD, (size_t)60 * n * 8, cudaMemcpyHostToDevice, c->stream));
+  int rc = cgks_set_state(c, tmp, hG ? tmp + 5 * n : nullptr, hD ? tmp + 20 * n : nullptr);
+  if (rc) return rc;
+  for (int s = 0; s < nsteps; s++) {
+    double dt;
+    rc = cgks_compute_dt(c, cfl, &dt); if (rc) return rc;
+    rc = cgks_step(c, dt); if (rc) return rc;
+  }
+  const double* Wc = c->W[c->cur];      // state layout equals the user layout: Q | G | D
+  if (oQ) CK(cudaMemcpyAsync(oQ, Wc, (size_t)5 * n * 8, cudaMemcpyDeviceToHost, c->stream));
+  if (oG) CK(cudaMemcpyAsync(oG, Wc + 5 * n, (size_t)15 * n * 8, cudaMemcpyDeviceToHost, c->stream));
+  if (oD) CK(cudaMemcpyAsync(oD, Wc + 20 * n, (size_t)60 * n * 8, cudaMemcpyDeviceToHost, c->stream));
+  return cgks_status(c);
+}

@@ -1,0 +1,316 @@
+// kernels_stage.cuh -- the three per-stage kernels of the S2O4 step:
+//   recon_kernel   compact reconstruction on the reference cell + GENO blend -> values/gradients at 24 face points
+//   flux_kernel    gas-kinetic flux + interface values at the 12 owned face Gauss points of each cell
+//   update_kernel  accumulate L, dL/dt, gradient and line sums; S2O4 stage combine
+// All index the mesh periodically and work on a slab of k-planes (see Slab).
+#pragma once
+#include "cgks_common.cuh"
+#include "gks_flux.cuh"
+#include "recon_gen.cuh"
+
+namespace cgks {
+
+struct ReconPrm { int nonlinear; double C, eps, inv_tanhC, gamma; };
+
+// ------------------------------------------------------------------------------------------------ reconstruction
+// Thread per (cell, variable).  PAPER.md:134-246 (Eq. 11-16), 250-300 (Eq. 17-19).
+template <bool CART>
+__global__ void __launch_bounds__(128) recon_kernel(Mesh m, Slab sl, const double* __restrict__ W, double* __restrict__ pv,
+                                                    double* __restrict__ chi_out, ReconPrm rp, int kA, long nthreads,
+                                                    int* __restrict__ flag) {
+  const long t = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= nthreads) return;
+  const int v = blockIdx.y;
+  const CellIdx x = cell_of(m, t, kA);
+  const long n = m.n;
+  if (v == 0) {      // physical admissibility of the incoming cell average (reported by cgks_status / cgks_compute_dt)
+    const double rho = W[x.c], mx = W[n + x.c], my = W[2 * n + x.c], mz = W[3 * n + x.c], E = W[4 * n + x.c];
+    if (!(rho > 0.0) || !(E - 0.5 * (mx * mx + my * my + mz * mz) / rho > 0.0)) atomicOr(flag, 1);
+  }
+  const int ii[3] = { wrap(x.i - 1, m.ni), x.i, wrap(x.i + 1, m.ni) };
+  const int jj[3] = { wrap(x.j - 1, m.nj), x.j, wrap(x.j + 1, m.nj) };
+  const int kk[3] = { wrap(x.k - 1, m.nk), x.k, wrap(x.k + 1, m.nk) };
+  double J[9], Ji[9];
+  if (!CART) {
+#pragma unroll
+    for (int q = 0; q < 9; q++) { J[q] = m.met[(MET_J0 + q) * n + x.c]; Ji[q] = m.met[(MET_J0INV + q) * n + x.c]; }
+  }
+  const double* q = W + (long)planeQ(v) * n;
+  const double* G0 = W + (long)planeG(v, 0) * n;
+  const double* G1 = W + (long)planeG(v, 1) * n;
+  const double* G2 = W + (long)planeG(v, 2) * n;
+  const double q0 = q[x.c];
+  double d[72];
+  // 18 neighbours: faces m = 2*axis + (0:+,1:-); edges e = 4*z0 + 2*(s1>0) + (s2>0)
+#pragma unroll
+  for (int nb = 0; nb < 18; nb++) {
+    int o[3] = { 0, 0, 0 }; int z0 = -1;
+    if (nb < 6) { o[nb / 2] = (nb % 2 == 0) ? 1 : -1; }
+    else {
+      const int e = nb - 6; z0 = e / 4;
+      const int o1 = (z0 == 0) ? 1 : 0, o2 = (z0 == 2) ? 1 : 2;
+      o[o1] = ((e >> 1) & 1) ? 1 : -1; o[o2] = (e & 1) ? 1 : -1;
+    }
+    const long cn = cell_at(m, ii[o[0] + 1], jj[o[1] + 1], kk[o[2] + 1]);
+    d[nb] = q[cn] - q0;
+    const double g0 = G0[cn], g1 = G1[cn], g2 = G2[cn];
+    double gr[3];      // (grad Q)' = J0^T grad Q with the target cell's J0
+    if (CART) { gr[0] = m.h[0] * g0; gr[1] = m.h[1] * g1; gr[2] = m.h[2] * g2; }
+    else {
+#pragma unroll
+      for (int a = 0; a < 3; a++) gr[a] = J[a] * g0 + J[3 + a] * g1 + J[6 + a] * g2;
+    }
+    if (nb < 6) { d[18 + 3 * nb] = 2.0 * gr[0]; d[18 + 3 * nb + 1] = 2.0 * gr[1]; d[18 + 3 * nb + 2] = 2.0 * gr[2]; }
+    else {
+      const int e = nb - 6;
+      d[36 + 2 * e] = gr[z0];
+      d[36 + 2 * e + 1] = (o[0] * gr[0] + o[1] * gr[1] + o[2] * gr[2]) * 0.70710678118654752440;
+    }
+  }
+  double Dl[12];
+#pragma unroll
+  for (int s = 0; s < 12; s++) { Dl[s] = W[(long)planeD(v, s) * n + x.c]; d[60 + s] = 3.0 * Dl[s]; }
+  double a[34];
+  recon_Md(d, a);
+  double chi = 1.0;
+  if (rp.nonlinear) {
+    // six linear polynomials (Eq. 15): normal slope = average difference, tangential = mean line difference
+    double la[3];
+#pragma unroll
+    for (int ax = 0; ax < 3; ax++) la[ax] = 0.25 * (Dl[4 * ax] + Dl[4 * ax + 1] + Dl[4 * ax + 2] + Dl[4 * ax + 3]);
+    double wsum = 0.0, bw[3] = { 0, 0, 0 };
+#pragma unroll
+    for (int mm = 0; mm < 6; mm++) {
+      double b[3] = { la[0], la[1], la[2] };
+      b[mm / 2] = (mm % 2 == 0) ? d[mm] : -d[mm];
+      const double IS = b[0] * b[0] + b[1] * b[1] + b[2] * b[2];
+      const double tt = IS + rp.eps, t2 = tt * tt;
+      const double wb = (1.0 / 6.0) / (t2 * t2 * tt);               // d_m/(IS_m + eps)^5
+      wsum += wb; bw[0] += wb * b[0]; bw[1] += wb * b[1]; bw[2] += wb * b[2];
+    }
+    // path function (readings G2, G3)
+    const double IS1 = recon_IS1(a), IS2 = recon_IS2(a), ISt = recon_IS34(a);
+    const double ISH = IS1 + IS2 + ISt;
+    const double rH = ISt / (ISH + rp.eps), rL = ISt / (IS1 + rp.eps);
+    const double aH = 1.0 + rH * rH, aL = 1.0 + rL * rL;
+    const double alpha = 2.0 * aH / (aH + aL);
+    chi = tanh(rp.C * alpha) * rp.inv_tanhC;
+    // Eq. 16 as one polynomial: chi P4 + (1-chi) sum_m omega_m P1_m
+    const double w1 = (1.0 - chi) / wsum;
+#pragma unroll
+    for (int b = 0; b < 3; b++) a[b] = chi * a[b] + w1 * bw[b];
+#pragma unroll
+    for (int b = 3; b < 34; b++) a[b] *= chi;
+  }
+  if (chi_out) chi_out[(long)v * n + x.c] = chi;
+  // values and gradients at the 24 face Gauss points, back-transformed
+  const long off = (long)slot_of(m, sl, x.k) * m.plane + x.ij;
+  double o[96];
+  recon_eval(a, o);
+#pragma unroll
+  for (int p = 0; p < 24; p++) {
+    double* dst = pv + (long)(p * 20) * sl.stride_pv + off;
+    dst[(long)v * sl.stride_pv] = q0 + o[4 * p];
+    double g[3];
+    if (CART) { g[0] = o[4 * p + 1] / m.h[0]; g[1] = o[4 * p + 2] / m.h[1]; g[2] = o[4 * p + 3] / m.h[2]; }
+    else {
+#pragma unroll
+      for (int r = 0; r < 3; r++) g[r] = Ji[r] * o[4 * p + 1] + Ji[3 + r] * o[4 * p + 2] + Ji[6 + r] * o[4 * p + 3];
+    }
+#pragma unroll
+    for (int r = 0; r < 3; r++) dst[(long)(5 + 3 * v + r) * sl.stride_pv] = g[r];
+  }
+}
+
+// ------------------------------------------------------------------------------------------------ flux
+// Thread per (cell, Gauss point q of the + face of AXIS); blockIdx.y = q.  PAPER.md:33-92, 330-352.
+// stage 2 stores only the time derivatives (reading T4).
+template <bool CART, int AXIS>
+__global__ void __launch_bounds__(128) flux_kernel(Mesh m, Slab sl, const double* __restrict__ W, const double* __restrict__ pv,
+                                                   double* __restrict__ fx, GasConst gc, double dt, int kA, long nthreads, int stage) {
+  const long t = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= nthreads) return;
+  const int q = blockIdx.y;
+  const CellIdx x = cell_of(m, t, kA);
+  // right cell
+  int ir = x.i, jr = x.j, kr = x.k;
+  if (AXIS == 0) ir = wrap(x.i + 1, m.ni); else if (AXIS == 1) jr = wrap(x.j + 1, m.nj); else kr = wrap(x.k + 1, m.nk);
+  const long offL = (long)slot_of(m, sl, x.k) * m.plane + x.ij;
+  const long offR = (long)slot_of(m, sl, kr) * m.plane + (long)jr * m.ni + ir;
+  const double* pL = pv + (long)((4 * (2 * AXIS) + q) * 20) * sl.stride_pv + offL;
+  const double* pR = pv + (long)((4 * (2 * AXIS + 1) + q) * 20) * sl.stride_pv + offR;
+  double WLg[5], WRg[5], gL[15], gR[15];
+#pragma unroll
+  for (int c = 0; c < 5; c++) { WLg[c] = pL[(long)c * sl.stride_pv]; WRg[c] = pR[(long)c * sl.stride_pv]; }
+#pragma unroll
+  for (int c = 0; c < 15; c++) { gL[c] = pL[(long)(5 + c) * sl.stride_pv]; gR[c] = pR[(long)(5 + c) * sl.stride_pv]; }
+  // positivity (reading R9, point-wise): a non-physical reconstructed state falls back to the cell average
+  {
+    const double eL = WLg[4] - 0.5 * (WLg[1] * WLg[1] + WLg[2] * WLg[2] + WLg[3] * WLg[3]) / WLg[0];
+    if (!(WLg[0] > 0.0) || !(eL > 0.0)) {
+#pragma unroll
+      for (int c = 0; c < 5; c++) WLg[c] = W[(long)c * m.n + x.c];
+#pragma unroll
+      for (int c = 0; c < 15; c++) gL[c] = 0.0;
+    }
+    const double eR = WRg[4] - 0.5 * (WRg[1] * WRg[1] + WRg[2] * WRg[2] + WRg[3] * WRg[3]) / WRg[0];
+    if (!(WRg[0] > 0.0) || !(eR > 0.0)) {
+      const long cr = cell_at(m, ir, jr, kr);
+#pragma unroll
+      for (int c = 0; c < 5; c++) WRg[c] = W[(long)c * m.n + cr];
+#pragma unroll
+      for (int c = 0; c < 15; c++) gR[c] = 0.0;
+    }
+  }
+  double WL[5], WR[5], SL[3][5], SR[3][5];
+  double fr[3][3];       // rows: n, t1, t2 (general meshes)
+  if (CART) {
+    // face frame = cyclic permutation of the axes: n = e_AXIS, t1 = e_(AXIS+1), t2 = e_(AXIS+2)
+    const int p0 = AXIS, p1 = (AXIS + 1) % 3, p2 = (AXIS + 2) % 3;
+    const int pm[3] = { p0, p1, p2 };
+    WL[0] = WLg[0]; WL[4] = WLg[4]; WR[0] = WRg[0]; WR[4] = WRg[4];
+#pragma unroll
+    for (int a = 0; a < 3; a++) { WL[1 + a] = WLg[1 + pm[a]]; WR[1 + a] = WRg[1 + pm[a]]; }
+#pragma unroll
+    for (int dd = 0; dd < 3; dd++) {
+      SL[dd][0] = gL[pm[dd]]; SL[dd][4] = gL[12 + pm[dd]]; SR[dd][0] = gR[pm[dd]]; SR[dd][4] = gR[12 + pm[dd]];
+#pragma unroll
+      for (int a = 0; a < 3; a++) { SL[dd][1 + a] = gL[3 * (1 + pm[a]) + pm[dd]]; SR[dd][1 + a] = gR[3 * (1 + pm[a]) + pm[dd]]; }
+    }
+  } else {
+    double A[3];
+#pragma unroll
+    for (int r = 0; r < 3; r++) { A[r] = m.met[(MET_AREA + 3 * AXIS + r) * m.n + x.c]; fr[1][r] = m.met[(MET_TAN + 3 * AXIS + r) * m.n + x.c]; }
+    const double S = sqrt(A[0] * A[0] + A[1] * A[1] + A[2] * A[2]);
+#pragma unroll
+    for (int r = 0; r < 3; r++) fr[0][r] = A[r] / S;
+    fr[2][0] = fr[0][1] * fr[1][2] - fr[0][2] * fr[1][1];
+    fr[2][1] = fr[0][2] * fr[1][0] - fr[0][0] * fr[1][2];
+    fr[2][2] = fr[0][0] * fr[1][1] - fr[0][1] * fr[1][0];
+#pragma unroll
+    for (int side = 0; side < 2; side++) {
+      const double* Wg = side ? WRg : WLg; const double* gg = side ? gR : gL;
+      double* Wl = side ? WR : WL; double (*Sx)[5] = side ? SR : SL;
+      Wl[0] = Wg[0]; Wl[4] = Wg[4];
+#pragma unroll
+      for (int a = 0; a < 3; a++) Wl[1 + a] = Wg[1] * fr[a][0] + Wg[2] * fr[a][1] + Wg[3] * fr[a][2];
+#pragma unroll
+      for (int dd = 0; dd < 3; dd++) {
+        double dg[5];
+#pragma unroll
+        for (int vv = 0; vv < 5; vv++) dg[vv] = gg[3 * vv] * fr[dd][0] + gg[3 * vv + 1] * fr[dd][1] + gg[3 * vv + 2] * fr[dd][2];
+        Sx[dd][0] = dg[0]; Sx[dd][4] = dg[4];
+#pragma unroll
+        for (int a = 0; a < 3; a++) Sx[dd][1 + a] = dg[1] * fr[a][0] + dg[2] * fr[a][1] + dg[3] * fr[a][2];
+      }
+    }
+  }
+  double out[6][5];      // Fn, Ft, VL, DL, VR, DR in the face frame
+  gks_flux_local(gc, dt, WL, SL, WR, SR, out[0], out[1], out[2], out[3], out[4], out[5]);
+  double* dst = fx + (long)((4 * AXIS + q) * 30) * sl.stride_fx + offL;
+#pragma unroll
+  for (int g = 0; g < 6; g++) {
+    if (stage == 2 && (g == 0 || g == 2 || g == 4)) continue;
+    double o3[3];
+    if (CART) {
+      const int p0 = AXIS, p1 = (AXIS + 1) % 3, p2 = (AXIS + 2) % 3;
+      o3[p0] = out[g][1]; o3[p1] = out[g][2]; o3[p2] = out[g][3];
+    } else {
+#pragma unroll
+      for (int r = 0; r < 3; r++) o3[r] = out[g][1] * fr[0][r] + out[g][2] * fr[1][r] + out[g][3] * fr[2][r];
+    }
+    dst[(long)(5 * g) * sl.stride_fx] = out[g][0];
+    dst[(long)(5 * g + 1) * sl.stride_fx] = o3[0];
+    dst[(long)(5 * g + 2) * sl.stride_fx] = o3[1];
+    dst[(long)(5 * g + 3) * sl.stride_fx] = o3[2];
+    dst[(long)(5 * g + 4) * sl.stride_fx] = out[g][4];
+  }
+}
+
+// ------------------------------------------------------------------------------------------------ update
+// Thread per (cell, variable).  Eq. 8-10 and the S2O4 combine.
+//   stage 1: Wstar = stage value at t_n + dt/2;  Wsave = { Q^n + dt L^n + dt^2/6 L_t^n,  G,D sums of V^n }
+//   stage 2: Wsave <- { Wsave.Q + dt^2/3 L_t^*,  Wsave.GD + dt * (G,D sums of Dt^*) }   (in place) = state at t_n+1
+template <bool CART>
+__global__ void __launch_bounds__(128) update_kernel(Mesh m, Slab sl, const double* __restrict__ fx, const double* __restrict__ Wcur,
+                                                     double* __restrict__ Wstar, double* __restrict__ Wsave, double dt,
+                                                     int kA, long nthreads, int stage) {
+  const long t = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= nthreads) return;
+  const int v = blockIdx.y;
+  const CellIdx x = cell_of(m, t, kA);
+  const long n = m.n;
+  const long offP = (long)slot_of(m, sl, x.k) * m.plane + x.ij;
+  double L = 0, Lt = 0, SG0[3] = { 0, 0, 0 }, SG1[3] = { 0, 0, 0 }, SD0[12], SD1[12];
+  double vol;
+  if (CART) vol = m.h[0] * m.h[1] * m.h[2]; else vol = m.met[MET_VOL * n + x.c];
+#pragma unroll
+  for (int ax = 0; ax < 3; ax++) {
+    int im = x.i, jm = x.j, km = x.k;
+    if (ax == 0) im = wrap(x.i - 1, m.ni); else if (ax == 1) jm = wrap(x.j - 1, m.nj); else km = wrap(x.k - 1, m.nk);
+    const long offM = (long)slot_of(m, sl, km) * m.plane + (long)jm * m.ni + im;
+    double Ap[3] = { 0, 0, 0 }, Am[3] = { 0, 0, 0 }, Sp, Sm;
+    if (CART) { Sp = Sm = vol / m.h[ax]; Ap[ax] = Sp; Am[ax] = Sm; }
+    else {
+      const long cm = cell_at(m, im, jm, km);
+#pragma unroll
+      for (int r = 0; r < 3; r++) { Ap[r] = m.met[(MET_AREA + 3 * ax + r) * n + x.c]; Am[r] = m.met[(MET_AREA + 3 * ax + r) * n + cm]; }
+      Sp = sqrt(Ap[0] * Ap[0] + Ap[1] * Ap[1] + Ap[2] * Ap[2]); Sm = sqrt(Am[0] * Am[0] + Am[1] * Am[1] + Am[2] * Am[2]);
+    }
+#pragma unroll
+    for (int q = 0; q < 4; q++) {
+      const double* fp = fx + (long)((4 * ax + q) * 30) * sl.stride_fx + offP;    // + face: this cell is the left side
+      const double* fm = fx + (long)((4 * ax + q) * 30) * sl.stride_fx + offM;    // - face: this cell is the right side
+      const double Ftp = fp[(long)(5 + v) * sl.stride_fx], Ftm = fm[(long)(5 + v) * sl.stride_fx];
+      const double Dp = fp[(long)(15 + v) * sl.stride_fx], Dm = fm[(long)(25 + v) * sl.stride_fx];
+      Lt -= 0.25 * (Ftp * Sp - Ftm * Sm);
+      SD1[4 * ax + q] = Dp - Dm;
+      if (CART) SG1[ax] += 0.25 * (Dp * Sp - Dm * Sm);
+      else {
+#pragma unroll
+        for (int r = 0; r < 3; r++) SG1[r] += 0.25 * (Dp * Ap[r] - Dm * Am[r]);
+      }
+      if (stage == 1) {
+        const double Fp = fp[(long)v * sl.stride_fx], Fm = fm[(long)v * sl.stride_fx];
+        const double Vp = fp[(long)(10 + v) * sl.stride_fx], Vm = fm[(long)(20 + v) * sl.stride_fx];
+        L -= 0.25 * (Fp * Sp - Fm * Sm);
+        SD0[4 * ax + q] = Vp - Vm;
+        if (CART) SG0[ax] += 0.25 * (Vp * Sp - Vm * Sm);
+        else {
+#pragma unroll
+          for (int r = 0; r < 3; r++) SG0[r] += 0.25 * (Vp * Ap[r] - Vm * Am[r]);
+        }
+      }
+    }
+  }
+  const double iv = 1.0 / vol;
+  Lt *= iv;
+#pragma unroll
+  for (int r = 0; r < 3; r++) SG1[r] *= iv;
+  if (stage == 1) {
+    L *= iv;
+#pragma unroll
+    for (int r = 0; r < 3; r++) SG0[r] *= iv;
+    const double qn = Wcur[(long)planeQ(v) * n + x.c];
+    Wstar[(long)planeQ(v) * n + x.c] = qn + 0.5 * dt * L + 0.125 * dt * dt * Lt;
+    Wsave[(long)planeQ(v) * n + x.c] = qn + dt * L + (1.0 / 6.0) * dt * dt * Lt;
+#pragma unroll
+    for (int r = 0; r < 3; r++) {
+      Wstar[(long)planeG(v, r) * n + x.c] = SG0[r] + 0.5 * dt * SG1[r];
+      Wsave[(long)planeG(v, r) * n + x.c] = SG0[r];
+    }
+#pragma unroll
+    for (int s = 0; s < 12; s++) {
+      Wstar[(long)planeD(v, s) * n + x.c] = SD0[s] + 0.5 * dt * SD1[s];
+      Wsave[(long)planeD(v, s) * n + x.c] = SD0[s];
+    }
+  } else {
+    Wsave[(long)planeQ(v) * n + x.c] += (1.0 / 3.0) * dt * dt * Lt;
+#pragma unroll
+    for (int r = 0; r < 3; r++) Wsave[(long)planeG(v, r) * n + x.c] += dt * SG1[r];
+#pragma unroll
+    for (int s = 0; s < 12; s++) Wsave[(long)planeD(v, s) * n + x.c] += dt * SD1[s];
+  }
+}
+
+}  // namespace cgks

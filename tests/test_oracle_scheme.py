@@ -211,12 +211,12 @@ def test_P11_double_shock_tube_no_overshoot():
 
 
 def test_bootstrap_of_derivative_dof():
-    """Reading S2: 4th-order central differences of cell averages; exact for a cubic in one direction is not
-    testable on a periodic box, so check the sine: error O(h^4)."""
+    """Reading S2: G from 4th-order central differences of cell averages (error O(h^4)); the four line differences
+    of an axis all get the axis value (error O(h^2) in D, regenerated by the scheme after the first step)."""
     errs = []
     for n in (8, 16):
         nodes, Q, G, D = inputs.sine_advection(n)
         s = ref.RefSolver(nodes, ref.make_params()); s.set_state(Q)
         _, Gb, Db = s.get_state()
         errs.append((np.abs(Gb - G).max(), np.abs(Db - D).max()))
-    assert errs[0][0] / errs[1][0] > 10 and errs[0][1] / errs[1][1] > 20
+    assert errs[0][0] / errs[1][0] > 10 and errs[0][1] / errs[1][1] > 3
