@@ -1,0 +1,273 @@
+#!/usr/bin/env python
+"""bench.py -- cell-updates/s per full S2O4 step of the CGKS-5 hot path on B200 (BASELINE.json metric).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--n 384] [--impl ours|reference]
+
+One "step" = cgks_compute_dt + cgks_step (two stages: reconstruction, GENO blend, gas-kinetic flux, update/combine)
+over the whole mesh.  Workload at N = 1: BASELINE.json configs[4], supersonic isotropic turbulence Ma_t = 1 on the
+periodic Cartesian 384^3 mesh (synthetic, seeded).  The path does not shard (north_star: one
+GPU, no collectives), so --gpus N runs N independent replicas ("replicas only", weak scaling).
+Prints ONE JSON line (rank 0).
+"""
+import argparse
+import json
+import math
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "cell-updates/s per S2O4 step (fp64)"
+UNIT = "cell-updates/s"
+# algorithmic fp64 flops of the dominant kernel (gas-kinetic flux) per face Gauss point: DESIGN.md section 7
+FLUX_FLOPS_PER_POINT = 4808.0
+FP64_PEAK_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12      # SMs x FP64 FMA lanes x 2 x max SM clock = 37.2
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=4)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--n", type=int, default=384, help="cells per direction (default: the 384^3 headline config)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+# ----------------------------------------------------------------------------------------------- clocks sampling
+class ClockSampler:
+    Q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
+        "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+
+    def __init__(self, index=0):
+        self.index = index; self.rows = []; self._stop = False; self.t = None
+
+    def _run(self):
+        while not self._stop:
+            try:
+                out = subprocess.run(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits"],
+                                     capture_output=True, text=True, timeout=5).stdout.strip()
+                if out:
+                    self.rows.append([x.strip() for x in out.split(",")])
+            except Exception:
+                pass
+            time.sleep(0.2)
+
+    def start(self):
+        self.t = threading.Thread(target=self._run, daemon=True); self.t.start()
+
+    def stop(self):
+        self._stop = True
+        if self.t:
+            self.t.join(timeout=6)
+        sm = []; mx = 0; reasons = set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx = max(mx, float(r[1]))
+                for nm, val in zip(names, r[3:7]):
+                    if val.lower().startswith("active"):
+                        reasons.add(nm)
+            except Exception:
+                pass
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": mx or None, "reasons": sorted(reasons), "samples": len(sm)}
+
+
+# ----------------------------------------------------------------------------------------------- oracle timing
+def oracle_sample(nsteps_hint=None):
+    """Times the CPU oracle, as it stands, on a bounded sample of the workload: the same generator (seed 5,
+    Ma_t = 1) on a periodic 32^3 mesh with k0 = 2, one S2O4 step per sample."""
+    from oracle import ref
+    from paper_2508_08965_b200 import inputs
+    n = 32
+    w = inputs.workload("iso_sup", n, 2.0)
+    s = ref.RefSolver(w["nodes"], ref.make_params(**w["params"], nonlinear=1))
+    s.set_state(w["Q"])
+    cores = os.cpu_count() or 1
+    try:
+        cores = len(os.sched_getaffinity(0))
+    except Exception:
+        pass
+    omp = os.environ.get("OMP_NUM_THREADS")
+    if omp:
+        cores = min(cores, int(omp))
+
+    def one():
+        t0 = time.perf_counter(); s.step(s.compute_dt(0.5)); return time.perf_counter() - t0
+    return s, n, cores, one
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    s, n, cores, one = oracle_sample()
+    for _ in range(min(args.warmup, 1)):
+        one()
+    t = 0.0
+    for _ in range(args.steps):
+        t += one()
+    cells = n ** 3
+    val = cells * args.steps / t
+    sample = "one S2O4 step per bench step on a periodic %d^3 mesh, same generator (seed 5, Ma_t=1, k0=2)" % n
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "iso_sup Ma_t=1.0 (oracle sample %d^3 of the 384^3 config)" % n},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# ----------------------------------------------------------------------------------------------- our arm
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2508_08965_b200 import binding, inputs
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
+    world = int(os.environ.get("WORLD_SIZE", "1")); rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    n = args.n
+    k0 = 8.0 if n >= 128 else 2.0
+    prm = inputs.iso_params(1.0, k0=k0)
+    nodes = torch.from_numpy(inputs.cartesian_nodes(n)).to(dev)
+    Q = inputs.iso_turbulence(n, 5 + rank, 1.0, k0, device=dev).contiguous()      # replicas: one seed per rank
+    Qhost = torch.empty(Q.shape, dtype=torch.float64, pin_memory=True); Qhost.copy_(Q)
+    Qout = torch.empty(Q.shape, dtype=torch.float64, pin_memory=True)
+    torch.cuda.empty_cache()
+    free, total = torch.cuda.mem_get_info(dev)
+    budget = int(free - (3 << 30))
+    solver = binding.Solver(nodes, binding.make_params(**prm, nonlinear=1), device=dev, budget_bytes=budget)
+    del nodes
+    solver.set_state(Q)
+    del Q
+    cells = n ** 3
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    def one_step():
+        solver.step(solver.compute_dt(0.5))
+
+    for _ in range(max(args.warmup, 3)):
+        one_step()
+    solver.status()
+    # ---- timed region: K steps, device resident, CUDA events on the launching stream -------------------------------
+    sampler = ClockSampler(local); sampler.start()
+    solver.set_profiling(True)
+    l0 = solver.launch_count()
+    barrier()
+    ev0 = torch.cuda.Event(enable_timing=True); ev1 = torch.cuda.Event(enable_timing=True)
+    ev0.record(torch.cuda.current_stream(dev))
+    for _ in range(args.steps):
+        one_step()
+    ev1.record(torch.cuda.current_stream(dev))
+    barrier()
+    ms = ev0.elapsed_time(ev1)
+    launches = solver.launch_count() - l0
+    clocks = sampler.stop()
+    kms = {k: solver.kernel_ms(k) for k in ("recon", "flux", "update", "cfl")}
+    solver.set_profiling(False)
+    solver.status()
+    chi = solver.chi()
+    chi_frac = float((chi < 0.99).double().mean().item())
+    del chi
+    tmax = torch.tensor([ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+    ms_max = float(tmax.item())
+    value = cells * world * args.steps / (ms_max * 1e-3)
+    # ---- end to end: host buffers through the C ABI, H2D + one step + D2H per bench step ---------------------------
+    e2e = None
+    if not args.no_e2e:
+        solver.run_host(Qhost, None, None, 0.5, 1, Qout)        # warm
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            solver.run_host(Qhost, None, None, 0.5, 1, Qout)    # synchronises inside (cgks_status)
+        barrier()
+        te = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(te, op=dist.ReduceOp.MAX)
+        nb = int(Qhost.numel() * 8)
+        e2e = {"value": cells * world * args.steps / float(te.item()), "unit": UNIT,
+               "h2d_bytes_per_step": nb, "d2h_bytes_per_step": nb}
+    # ---- roofline of the dominant kernel (gas-kinetic flux) ---------------------------------------------------------
+    peak_meas = binding.fp64_peak_tflops(dev) if rank == 0 else None
+    fms, fnl = kms["flux"]
+    roof = None
+    if fnl > 0:
+        # every flux launch covers 4 Gauss points of one face direction of its cells; summed over the launches of the
+        # timed region the points are 12 per cell per stage (+ the recomputed halo plane of each slab, counted in fnl)
+        pts_per_step = 2 * 12 * cells * slab_overhead(solver, n)
+        flops = FLUX_FLOPS_PER_POINT * pts_per_step * args.steps
+        ach = flops / (fms * 1e-3) / 1e12
+        roof = {"bound": "alu", "kernel": "flux_kernel", "achieved": ach, "peak": FP64_PEAK_NOMINAL_TFLOPS, "unit": "TFLOP/s",
+                "frac": ach / FP64_PEAK_NOMINAL_TFLOPS, "traffic": None,
+                "peak_source": "derived: 148 SMs x 64 FP64 FMA lanes x 2 x 1.965 GHz (DESIGN.md section 7); "
+                               "MEASURED_PEAKS.json has no FP64 entry",
+                "peak_dfma_microbench": peak_meas, "avg_launch_ms": fms / fnl, "launches": fnl,
+                "share_of_step": fms / (ms if ms > 0 else 1.0),
+                "kernel_ms_per_step": {k: v[0] / args.steps for k, v in kms.items()}}
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+            "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "iso_sup: supersonic isotropic turbulence Ma_t=1.0, periodic Cartesian %d^3 (BASELINE.json configs[4])" % n,
+                       "cells": cells, "nonlinear": 1, "cfl": 0.5, "parallelism": "replicas only" if world > 1 else "single GPU",
+                       "l2": "inputs larger than L2 (state %.1f GB per buffer)" % (80 * cells * 8 / 1e9),
+                       "slab_depth": solver_slab(solver), "chi_below_0.99_fraction": chi_frac},
+            "clocks": clocks, "gpu_launches": launches, "e2e": e2e, "roofline": roof}
+    if rank == 0:
+        if not args.no_cpu_baseline and world == 1:
+            line["cpu_baseline"] = cpu_baseline()
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def solver_slab(solver):
+    from paper_2508_08965_b200 import binding
+    return int(binding.lib().cgks_slab_depth(solver._h))
+
+
+def slab_overhead(solver, n):
+    """Flux launches cover one extra k-plane per slab (recomputed halo) unless the whole mesh is resident."""
+    S = solver_slab(solver)
+    if S >= n:
+        return 1.0
+    nchunks = math.ceil(n / S)
+    return (n + nchunks) / n
+
+
+def cpu_baseline():
+    s, n, cores, one = oracle_sample()
+    one()
+    t = 0.0; k = 0
+    while t < 10.0 and k < 8:
+        t += one(); k += 1
+    return {"value": n ** 3 * k / t, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": "%d S2O4 steps on a periodic %d^3 mesh, same generator (seed 5, Ma_t=1, k0=2), after 1 warm step" % (k, n)}
+
+
+if __name__ == "__main__":
+    a = parse()
+    if a.impl == "reference":
+        run_reference(a)
+    else:
+        run_ours(a)

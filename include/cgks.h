@@ -86,6 +86,9 @@ int cgks_status(cgks_ctx*);
 int cgks_run_host(cgks_ctx*, const double* h_Q, const double* h_G, const double* h_D, double cfl, int nsteps,
                   double* h_Q_out, double* h_G_out, double* h_D_out);
 
+/* Depth in k-planes of the slab pipeline chosen by cgks_create from the workspace size (nk: whole mesh resident). */
+int cgks_slab_depth(const cgks_ctx*);
+
 /* Number of kernels launched by the library on this context so far (for bench.py's gpu_launches). */
 long cgks_launch_count(const cgks_ctx*);
 
@@ -98,6 +101,17 @@ int cgks_kernel_ms(const cgks_ctx*, int which, double* ms, long* launches);
 /* Debug/testing taps (device pointers, valid until the next cgks_step): reconstructed face values of slab-resident
    cells are not exposed; instead this returns chi of the last reconstruction, [5][nk][nj][ni], copied to d_chi. */
 int cgks_get_chi(cgks_ctx*, double* d_chi);
+
+/* Test tap: runs the reconstruction (and, if d_fx != NULL, the flux kernels with step size dt, stage 1) on the
+   CURRENT state and copies the slab buffers out: d_pv [480][N] (plane (4m+q)*20 + c: c = v value, 5+3v+r physical
+   gradient; NO positivity fallback applied), d_fx [360][N] (plane (4ax+q)*30 + c: Fn, Ft, VL, DtL, VR, DtR).
+   Needs the whole mesh resident (CGKS_ENOMEM otherwise).  The state is not modified. */
+int cgks_debug_stage(cgks_ctx*, double dt, double* d_pv, double* d_fx);
+
+/* Measures the device's FP64 FMA throughput with a register-resident DFMA micro-benchmark (8 independent chains
+   per thread, 148*8 blocks of 256 threads) on `cuda_stream`; TFLOP/s (FMA = 2 flops) to *tflops (host).
+   The only call that allocates device memory itself (8 bytes, freed before returning). */
+int cgks_fp64_peak(void* cuda_stream, double* tflops);
 
 int cgks_destroy(cgks_ctx*);
 const char* cgks_last_error(const cgks_ctx*);

@@ -695,6 +695,13 @@ static void flux_all(cgks_ref_ctx* c, double dt) {
   }
 }
 
+/* test tap: reconstruct + flux of the current state; fx [3][ncell][4][30] */
+int cgks_ref_debug_flux(cgks_ref_ctx* c, double dt, double* fx) {
+  reconstruct_all(c); flux_all(c, dt);
+  memcpy(fx, c->fx, sizeof(double) * 3 * c->n * 4 * 30);
+  return 0;
+}
+
 void cgks_ref_s2o4_stage1(double qn, double L, double Lt, double dt, double* qstar) {
   *qstar = qn + 0.5 * dt * L + 0.125 * dt * dt * Lt;                       /* PAPER.md:322 */
 }

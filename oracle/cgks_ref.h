@@ -61,6 +61,8 @@ void   cgks_ref_smoothness(const double* a, double* IS4);
 /* reconstruct every cell of the current state: pv [ncell][24][20] = (5 values, 15 physical
    gradient comps [v][dir]); chi [5][ncell] */
 int    cgks_ref_reconstruct(cgks_ref_ctx*, double* pv, double* chi);
+/* reconstruct + flux of the current state: fx [3][ncell][4][30] = Fn, Ft, VL, DtL, VR, DtR per owned face point */
+int    cgks_ref_debug_flux(cgks_ref_ctx*, double dt, double* fx);
 /* gas-kinetic solver at one face Gauss point, global frame in/out.
    WL/WR[5], gL/gR[5][3] physical gradients, n,t1 unit vectors (t2 = n x t1).
    out[30] = Fn[5], Ft[5] (normal flux and its time derivative), VL[5], DtL[5], VR[5], DtR[5] */

@@ -50,6 +50,7 @@ def lib():
         L.cgks_ref_recon_reference.argtypes = [C.POINTER(Params)] + [_dp] * 7
         L.cgks_ref_smoothness.argtypes = [_dp, _dp]
         L.cgks_ref_reconstruct.argtypes = [C.c_void_p, _dp, _dp]
+        L.cgks_ref_debug_flux.argtypes = [C.c_void_p, C.c_double, _dp]
         L.cgks_ref_flux_point.argtypes = [C.POINTER(Params), C.c_double] + [_dp] * 7
         L.cgks_ref_moments.argtypes = [C.c_double, C.c_double, _dp, _dp, _dp]
         L.cgks_ref_microslope.argtypes = [_dp] + [C.c_double] * 5 + [_dp]
@@ -171,6 +172,11 @@ class RefSolver:
         pv = np.zeros((self.nk, self.nj, self.ni, NGP, 20)); chi = np.zeros((5, self.nk, self.nj, self.ni))
         lib().cgks_ref_reconstruct(self._h, _p(pv), _p(chi))
         return pv, chi
+
+    def debug_flux(self, dt):
+        fx = np.zeros((3, self.nk, self.nj, self.ni, 4, 30))
+        lib().cgks_ref_debug_flux(self._h, float(dt), _p(fx))
+        return fx
 
     def geometry(self):
         vol = np.zeros((self.nk, self.nj, self.ni)); J0 = np.zeros((self.nk, self.nj, self.ni, 3, 3))

@@ -49,9 +49,12 @@ def lib():
         L.cgks_status.argtypes = [_vp]
         L.cgks_run_host.argtypes = [_vp, _vp, _vp, _vp, C.c_double, C.c_int, _vp, _vp, _vp]
         L.cgks_launch_count.argtypes = [_vp]; L.cgks_launch_count.restype = C.c_long
+        L.cgks_slab_depth.argtypes = [_vp]
         L.cgks_set_profiling.argtypes = [_vp, C.c_int]
         L.cgks_kernel_ms.argtypes = [_vp, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_long)]
         L.cgks_get_chi.argtypes = [_vp, _vp]
+        L.cgks_debug_stage.argtypes = [_vp, C.c_double, _vp, _vp]
+        L.cgks_fp64_peak.argtypes = [_vp, C.POINTER(C.c_double)]
         L.cgks_destroy.argtypes = [_vp]
         L.cgks_last_error.argtypes = [_vp]; L.cgks_last_error.restype = C.c_char_p
         L.cgks_version.restype = C.c_char_p
@@ -72,6 +75,17 @@ def workspace_bytes(ni, nj, nk, budget_bytes=0):
     return out.value
 
 
+def fp64_peak_tflops(device="cuda:0"):
+    """DFMA micro-benchmark (cgks_fp64_peak): measured FP64 FMA throughput of the device in TFLOP/s."""
+    out = C.c_double(0.0)
+    with torch.cuda.device(device):
+        st = torch.cuda.current_stream()
+        rc = lib().cgks_fp64_peak(_vp(st.cuda_stream), C.byref(out))
+    if rc:
+        raise CgksError(rc, "cgks_fp64_peak")
+    return out.value
+
+
 def _dev(a, device):
     if a is None:
         return None
@@ -89,7 +103,7 @@ class Solver:
 
     nodes (3, nk+1, nj+1, ni+1); Q (5, nk, nj, ni); G (5, 3, nk, nj, ni); D (5, 12, nk, nj, ni)."""
 
-    def __init__(self, nodes, params, device="cuda:0", budget_bytes=0):
+    def __init__(self, nodes, params, device="cuda:0", budget_bytes=0, workspace_nbytes=None):
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2508_08965_b200 needs a CUDA device (no CPU fallback)")
         self.device = torch.device(device)
@@ -99,7 +113,7 @@ class Solver:
         self.nk, self.nj, self.ni = (int(s) - 1 for s in nodes.shape[1:])
         self.n = self.ni * self.nj * self.nk
         self.params = params if isinstance(params, cgks_params) else make_params(**params)
-        nbytes = workspace_bytes(self.ni, self.nj, self.nk, budget_bytes)
+        nbytes = workspace_nbytes or workspace_bytes(self.ni, self.nj, self.nk, budget_bytes)
         with torch.cuda.device(self.device):
             self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
             self.stream = torch.cuda.current_stream(self.device)
@@ -159,6 +173,14 @@ class Solver:
         def hp(t):
             return None if t is None else _vp(t.data_ptr())
         self._check(lib().cgks_run_host(self._h, hp(Q), hp(G), hp(D), float(cfl), int(nsteps), hp(out_Q), hp(out_G), hp(out_D)))
+
+    def debug_stage(self, dt=None):
+        """Test tap: (pv [24][20][nk][nj][ni], fx [12][30][nk][nj][ni] or None) of the current state."""
+        s = (self.nk, self.nj, self.ni)
+        pv = torch.empty((24, 20) + s, dtype=torch.float64, device=self.device)
+        fx = None if dt is None else torch.empty((12, 30) + s, dtype=torch.float64, device=self.device)
+        self._check(lib().cgks_debug_stage(self._h, 0.0 if dt is None else float(dt), _ptr(pv), _ptr(fx)))
+        return pv, fx
 
     def launch_count(self):
         return int(lib().cgks_launch_count(self._h))

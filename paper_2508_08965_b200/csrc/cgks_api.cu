@@ -59,6 +59,7 @@ static int cuda_fail(cgks_ctx* c, cudaError_t e, const char* where) {
 extern "C" const char* cgks_version(void) { return "cgks-b200 0.1 (sm_100a, fp64)"; }
 extern "C" const char* cgks_last_error(const cgks_ctx* c) { return c ? c->err.c_str() : "null context"; }
 extern "C" long cgks_launch_count(const cgks_ctx* c) { return c ? c->launches : 0; }
+extern "C" int cgks_slab_depth(const cgks_ctx* c) { return c ? c->S : 0; }
 
 static size_t fixed_bytes(long n, bool with_metrics) {
   size_t b = 3 * state_bytes(n) + align_up((size_t)5 * n * 8) + align_up(64);
@@ -314,6 +315,29 @@ extern "C" int cgks_step(cgks_ctx* c, double dt) {
   return CGKS_OK;
 }
 
+// ---- test taps: reconstruction / flux of the CURRENT state, whole mesh resident only ------------------------------
+extern "C" int cgks_debug_stage(cgks_ctx* c, double dt, double* d_pv, double* d_fx) {
+  if (!c) return CGKS_EINVAL;
+  const Mesh& m = c->mesh;
+  if (c->S < m.nk) return fail(c, CGKS_ENOMEM, "debug taps need the whole mesh resident");
+  ReconPrm rp{ c->prm.nonlinear, c->prm.geno_C, c->prm.geno_eps, 1.0 / tanh(c->prm.geno_C), c->prm.gamma };
+  Slab sl; sl.kbase = 0; sl.slots_pv = c->slots_pv; sl.slots_fx = c->slots_fx;
+  sl.stride_pv = (long)c->slots_pv * m.plane; sl.stride_fx = (long)c->slots_fx * m.plane;
+  const long nt = m.n;
+  dim3 grid((unsigned)((nt + TPB - 1) / TPB), 5);
+  const double* Win = c->W[c->cur];
+  if (m.cart) recon_kernel<true><<<grid, TPB, 0, c->stream>>>(m, sl, Win, c->pv, c->chi, rp, 0, nt, c->d_flags + 3);
+  else recon_kernel<false><<<grid, TPB, 0, c->stream>>>(m, sl, Win, c->pv, c->chi, rp, 0, nt, c->d_flags + 3);
+  c->launches++;
+  if (d_pv) CK(cudaMemcpyAsync(d_pv, c->pv, (size_t)NPV * m.n * 8, cudaMemcpyDeviceToDevice, c->stream));
+  if (d_fx) {
+    if (m.cart) launch_flux<true>(c, sl, Win, dt, 0, m.nk, 1); else launch_flux<false>(c, sl, Win, dt, 0, m.nk, 1);
+    CK(cudaMemcpyAsync(d_fx, c->fx, (size_t)NFX * m.n * 8, cudaMemcpyDeviceToDevice, c->stream));
+  }
+  CK(cudaGetLastError());
+  return CGKS_OK;
+}
+
 extern "C" int cgks_set_profiling(cgks_ctx* c, int on) {
   if (!c) return CGKS_EINVAL;
   c->profiling = on ? 1 : 0;
@@ -325,6 +349,43 @@ extern "C" int cgks_kernel_ms(const cgks_ctx* c, int which, double* ms, long* la
   if (!c || which < 0 || which >= KC_N) return CGKS_EINVAL;
   if (ms) *ms = c->ms[which];
   if (launches) *launches = c->nl[which];
+  return CGKS_OK;
+}
+
+// ---- FP64 FMA peak micro-benchmark (roofline denominator check) ------------------------------------------------------
+__global__ void __launch_bounds__(256) dfma_peak_kernel(double* out, int iters, double a, double b) {
+  double x0 = threadIdx.x * 1e-3, x1 = x0 + 1, x2 = x0 + 2, x3 = x0 + 3, x4 = x0 + 4, x5 = x0 + 5, x6 = x0 + 6, x7 = x0 + 7;
+  for (int i = 0; i < iters; i++) {
+#pragma unroll
+    for (int u = 0; u < 8; u++) {
+      x0 = fma(x0, a, b); x1 = fma(x1, a, b); x2 = fma(x2, a, b); x3 = fma(x3, a, b);
+      x4 = fma(x4, a, b); x5 = fma(x5, a, b); x6 = fma(x6, a, b); x7 = fma(x7, a, b);
+    }
+  }
+  const double s = x0 + x1 + x2 + x3 + x4 + x5 + x6 + x7;
+  if (s == 12345.678) out[0] = s;      // never true; keeps the chains alive
+}
+
+extern "C" int cgks_fp64_peak(void* stream, double* tflops) {
+  if (!tflops) return CGKS_EINVAL;
+  cgks_ctx* c = nullptr;
+  cudaStream_t st = (cudaStream_t)stream;
+  double* d = nullptr;
+  CK(cudaMalloc(&d, 8));
+  const int blocks = 148 * 8, iters = 4096;
+  cudaEvent_t a, b; cudaEventCreate(&a); cudaEventCreate(&b);
+  double best = 0;
+  for (int rep = 0; rep < 5; rep++) {
+    cudaEventRecord(a, st);
+    dfma_peak_kernel<<<blocks, 256, 0, st>>>(d, iters, 0.999999, 1e-7);
+    cudaEventRecord(b, st);
+    if (cudaEventSynchronize(b) != cudaSuccess) { cudaFree(d); return CGKS_ECUDA; }
+    float ms = 0; cudaEventElapsedTime(&ms, a, b);
+    const double fl = 2.0 * 64.0 * iters * 256.0 * blocks;
+    if (rep > 0 && fl / (ms * 1e-3) * 1e-12 > best) best = fl / (ms * 1e-3) * 1e-12;
+  }
+  cudaEventDestroy(a); cudaEventDestroy(b); cudaFree(d);
+  *tflops = best;
   return CGKS_OK;
 }
 

@@ -130,34 +130,58 @@ def iso_params(Ma_t, Re_lambda=72.0, k0=8.0, gamma=1.4, Pr=0.7):
     return dict(gamma=gamma, Pr=Pr, mu_ref=mu_ref, visc_omega=0.76, T_ref=p / 1.0, tau_c1=0.0, tau_c2=5.0)
 
 
-def iso_turbulence(n, seed, Ma_t, k0=8.0, gamma=1.4):
+def iso_turbulence(n, seed, Ma_t, k0=8.0, gamma=1.4, device=None):
     """Solenoidal random-phase velocity with E(k) ~ k^4 exp(-2 k^2/k0^2) on the periodic n^3 mesh of [0,2pi]^3,
-    rescaled to <u.u>^(1/2) = 1; rho = 1, p = 1/(gamma Ma_t^2)."""
+    rescaled to <u.u>^(1/2) = 1; rho = 1, p = 1/(gamma Ma_t^2).
+    With `device` (a torch device) the FFTs run there and a torch tensor on that device is returned (same recipe and
+    seed, results equal to the numpy path to round-off); used for the 384^3 bench input."""
     rng = np.random.Generator(np.random.PCG64(seed))
     noise = rng.standard_normal((3, n, n, n))
-    uh = np.fft.fftn(noise, axes=(1, 2, 3))
-    mag = np.abs(uh); mag[mag == 0] = 1.0
+    if device is not None:
+        import torch
+        xp = torch
+        noise = torch.from_numpy(noise).to(device)
+        fftn = lambda a: torch.fft.fftn(a, dim=(1, 2, 3))
+        ifftn = lambda a: torch.fft.ifftn(a, dim=(1, 2, 3))
+        kk = torch.fft.fftfreq(n, 1.0 / n, dtype=torch.float64, device=device)
+        KZ, KY, KX = torch.meshgrid(kk, kk, kk, indexing="ij")
+        stack, where, sqrt, exp, absf, real = torch.stack, torch.where, torch.sqrt, torch.exp, torch.abs, torch.real
+        one = lambda a: torch.ones_like(a)
+    else:
+        xp = np
+        fftn = lambda a: np.fft.fftn(a, axes=(1, 2, 3))
+        ifftn = lambda a: np.fft.ifftn(a, axes=(1, 2, 3))
+        kk = np.fft.fftfreq(n, 1.0 / n)
+        KZ, KY, KX = np.meshgrid(kk, kk, kk, indexing="ij")
+        stack, where, sqrt, exp, absf, real = np.stack, np.where, np.sqrt, np.exp, np.abs, np.real
+        one = lambda a: np.ones_like(a)
+    uh = fftn(noise)
+    del noise
+    mag = absf(uh); mag = where(mag == 0, one(mag), mag)
     uh = uh / mag                                       # unit modulus, random phase, Hermitian symmetric
-    kk = np.fft.fftfreq(n, 1.0 / n)
-    KZ, KY, KX = np.meshgrid(kk, kk, kk, indexing="ij")
-    kvec = np.stack([KX, KY, KZ]); k2 = (kvec ** 2).sum(0); k2s = np.where(k2 == 0, 1.0, k2)
+    del mag
+    kvec = stack([KX, KY, KZ]); k2 = (kvec ** 2).sum(0); k2s = where(k2 == 0, one(k2), k2)
     uh = uh - kvec * (kvec * uh).sum(0) / k2s           # solenoidal projection
-    kmag = np.sqrt(k2s)
-    Ek = kmag ** 4 * np.exp(-2.0 * k2 / (k0 * k0))
-    amp = np.sqrt(Ek / (2.0 * math.pi * k2s)); amp[k2 == 0] = 0.0
-    nrm = np.sqrt((np.abs(uh) ** 2).sum(0)); nrm[nrm == 0] = 1.0
+    Ek = k2s ** 2 * exp(-2.0 * k2 / (k0 * k0))
+    amp = sqrt(Ek / (2.0 * math.pi * k2s)); amp = where(k2 == 0, 0.0 * amp, amp)
+    nrm = sqrt((absf(uh) ** 2).sum(0)); nrm = where(nrm == 0, one(nrm), nrm)
     uh = uh / nrm * amp
-    u = np.real(np.fft.ifftn(uh, axes=(1, 2, 3)))
-    u /= math.sqrt((u ** 2).sum(0).mean())
-    rho = np.ones((n, n, n)); p = np.full((n, n, n), 1.0 / (gamma * Ma_t * Ma_t))
-    # velocity array order (x, y, z) with array axes (k, j, i) = (z, y, x)
-    return prim_to_cons(rho, u[0], u[1], u[2], p, gamma)
+    del nrm, amp, Ek, kvec
+    u = real(ifftn(uh))
+    del uh
+    u = u / math.sqrt(float((u ** 2).sum(0).mean()))
+    pval = 1.0 / (gamma * Ma_t * Ma_t)
+    # velocity components (x, y, z) = u[0], u[1], u[2]; array axes (k, j, i) = (z, y, x)
+    ke = 0.5 * (u[0] * u[0] + u[1] * u[1] + u[2] * u[2])
+    return stack([one(ke), u[0], u[1], u[2], pval / (gamma - 1.0) + ke])
 
 
 # ----------------------------------------------------------------------------- named workloads
-def workload(name, n=None):
+def workload(name, n=None, k0=None):
     """Returns dict(nodes, Q, G, D, params, nonlinear, cfl, steps) for the five BASELINE.json configs.
-    G, D are None when the derivative dof are bootstrapped by cgks_set_state."""
+    G, D are None when the derivative dof are bootstrapped by cgks_set_state.
+    For the turbulence cases k0 (spectrum peak, BASELINE.json: 8) may be lowered on small test meshes so that the
+    field keeps a resolution comparable to the full-size workload (384^3 with k0 = 8 has 48 cells per peak wavelength)."""
     if name == "sine":
         n = n or 16
         nodes, Q, G, D = sine_advection(n)
@@ -176,10 +200,12 @@ def workload(name, n=None):
         return dict(nodes=nodes, Q=free_stream((n, n, n)), G=None, D=None, params=tgv_params(), nonlinear=1, cfl=0.5, steps=100)
     if name == "iso_sub":
         n = n or 128
-        return dict(nodes=cartesian_nodes(n), Q=iso_turbulence(n, 4, 0.5), G=None, D=None, params=iso_params(0.5),
+        k0 = k0 or 8.0
+        return dict(nodes=cartesian_nodes(n), Q=iso_turbulence(n, 4, 0.5, k0), G=None, D=None, params=iso_params(0.5, k0=k0),
                     nonlinear=1, cfl=0.5, steps=500)
     if name == "iso_sup":
         n = n or 384
-        return dict(nodes=cartesian_nodes(n), Q=iso_turbulence(n, 5, 1.0), G=None, D=None, params=iso_params(1.0),
+        k0 = k0 or 8.0
+        return dict(nodes=cartesian_nodes(n), Q=iso_turbulence(n, 5, 1.0, k0), G=None, D=None, params=iso_params(1.0, k0=k0),
                     nonlinear=1, cfl=0.5, steps=100)
     raise KeyError(name)

@@ -8,11 +8,16 @@ from paper_2508_08965_b200 import inputs
 
 def field_errors(gpu, orc, nodes, Qref):
     """Relative L-infinity error per field (80 planes): max|gpu-oracle| / max(|oracle|_inf, delta_f) with the floors
-    delta_f = 1e-3 |Q_v|_inf (D planes), 1e-3 |Q_v|_inf / h_min (G planes), 1e-3 |rho|_inf max|U| (momentum planes)."""
+    delta_f = 1e-3 |Q_v|_inf (D planes), 1e-3 |Q_v|_inf / h_min (G planes), 1e-3 |rho|_inf max(|U|+c) (momentum planes;
+    for a momentum variable |Q_v|_inf in the D and G floors is replaced by max(|Q_v|_inf, momentum floor)).
+    The floors keep fields that are identically ~0 (free-stream derivatives, transverse momenta of 1-D flows)
+    from turning round-off noise into O(1) 'relative' errors."""
     Qg, Gg, Dg = gpu; Qo, Go, Do = orc
     hmin = min(np.abs(np.diff(nodes[0], axis=2)).min(), np.abs(np.diff(nodes[1], axis=1)).min(), np.abs(np.diff(nodes[2], axis=0)).min())
     qinf = [np.abs(Qref[v]).max() for v in range(5)]
-    umax = max(np.abs(Qref[1:4] / Qref[0]).max(), 1e-300)
+    rho = Qref[0]; U = Qref[1:4] / rho
+    pres = 0.4 * (Qref[4] - 0.5 * rho * (U ** 2).sum(0))
+    umax = (np.sqrt((U ** 2).sum(0)) + np.sqrt(1.4 * pres / rho)).max()      # velocity scale |U| + c
     mom_floor = 1e-3 * qinf[0] * umax
     errs = {}
     for v in range(5):
@@ -26,8 +31,8 @@ def field_errors(gpu, orc, nodes, Qref):
     return errs
 
 
-def build_case(name, n=None, nonlinear=None):
-    w = inputs.workload(name, n)
+def build_case(name, n=None, nonlinear=None, k0=None):
+    w = inputs.workload(name, n, k0)
     if nonlinear is not None:
         w["nonlinear"] = nonlinear
     return w
