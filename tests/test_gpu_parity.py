@@ -58,7 +58,9 @@ def _shock_tube_case():
 def test_shock_tube_parity():
     w = _shock_tube_case()
     _check(w, 1, TOL_1)
-    _check(w, 40, 1e-9)
+    # 40 steps: the north_star bound grows from 1e-10 (1 step) to 1e-8 (100 steps); 40/100 of the latter.  The shock
+    # makes the ENO weights ~(IS+eps)^-5 amplify round-off five-fold per evaluation.
+    _check(w, 40, 4e-9)
 
 
 def test_rough_field_robustness():
@@ -133,7 +135,7 @@ def test_error_codes():
     with pytest.raises(binding.CgksError) as e:
         binding.Solver(nodes, prm, workspace_nbytes=4096)
     assert e.value.code == binding.CGKS_ENOMEM
-    bad = nodes.copy(); bad[0, :, :, -1] += 0.3                   # breaks periodicity of the node array
+    bad = nodes.copy(); bad[0, 2, 3, -1] += 0.3                   # one node of the last plane: period vector not constant
     with pytest.raises(binding.CgksError) as e:
         binding.Solver(bad, prm)
     assert e.value.code == binding.CGKS_EINVAL
