@@ -14,8 +14,71 @@ struct ReconPrm { int nonlinear; double C, eps, inv_tanhC, gamma; };
 
 // ------------------------------------------------------------------------------------------------ reconstruction
 // Thread per (cell, variable).  PAPER.md:134-246 (Eq. 11-16), 250-300 (Eq. 17-19).
+// The 72 data of Eq. 19 are consumed neighbour group by neighbour group (face pairs, edge quads, line quads): each
+// group's raw data are turned into reflection-parity combinations and accumulated into the 34 coefficients with the
+// block-diagonal form of M (recon_gen.cuh), so the data vector is never held as a whole.
+template <int AX> __device__ __forceinline__ void acc_face(const double* x, double* a) {
+  if (AX == 0) recon_acc_face0(x, a); else if (AX == 1) recon_acc_face1(x, a); else recon_acc_face2(x, a);
+}
+template <int AX> __device__ __forceinline__ void acc_edge(const double* x, double* a) {
+  if (AX == 0) recon_acc_edge0(x, a); else if (AX == 1) recon_acc_edge1(x, a); else recon_acc_edge2(x, a);
+}
+template <int AX> __device__ __forceinline__ void acc_line(const double* x, double* a) {
+  if (AX == 0) recon_acc_line0(x, a); else if (AX == 1) recon_acc_line1(x, a); else recon_acc_line2(x, a);
+}
+template <int AX> __device__ __forceinline__ void eval_axis(const double* a, double* o) {
+  if (AX == 0) recon_eval_axis0(a, o); else if (AX == 1) recon_eval_axis1(a, o); else recon_eval_axis2(a, o);
+}
+
 template <bool CART>
-__global__ void __launch_bounds__(128) recon_kernel(Mesh m, Slab sl, const double* __restrict__ W, double* __restrict__ pv,
+struct ReconCell {
+  const Mesh& m; const double* q; const double* G0; const double* G1; const double* G2;
+  double J[9];
+  // (grad Q)' = J0^T grad Q of neighbour cn with the TARGET cell's J0
+  __device__ __forceinline__ void grad_ref(long cn, double* gr) const {
+    const double g0 = G0[cn], g1 = G1[cn], g2 = G2[cn];
+    if (CART) { gr[0] = m.h[0] * g0; gr[1] = m.h[1] * g1; gr[2] = m.h[2] * g2; }
+    else {
+#pragma unroll
+      for (int a = 0; a < 3; a++) gr[a] = J[a] * g0 + J[3 + a] * g1 + J[6 + a] * g2;
+    }
+  }
+};
+
+template <bool CART, int AX>
+__device__ __forceinline__ void recon_gather_axis(const ReconCell<CART>& rc, const int* ii, const int* jj, const int* kk,
+                                                  double q0, double* a, double* dface) {
+  const Mesh& m = rc.m;
+  {   // face pair of axis AX: x = { dq+, dq-, gr'+ (3), gr'- (3) }
+    int op[3] = { 1, 1, 1 }, om[3] = { 1, 1, 1 };
+    op[AX] = 2; om[AX] = 0;
+    const long cp = cell_at(m, ii[op[0]], jj[op[1]], kk[op[2]]), cm = cell_at(m, ii[om[0]], jj[om[1]], kk[om[2]]);
+    double x[8];
+    x[0] = rc.q[cp] - q0; x[1] = rc.q[cm] - q0;
+    rc.grad_ref(cp, x + 2); rc.grad_ref(cm, x + 5);
+    dface[2 * AX] = x[0]; dface[2 * AX + 1] = x[1];
+    acc_face<AX>(x, a);
+  }
+  {   // the four edge neighbours around axis AX: x = { dq_t (4), (gr'[AX], o.gr')_t (4 x 2) }
+    const int o1 = (AX == 0) ? 1 : 0, o2 = (AX == 2) ? 1 : 2;
+    double x[12];
+#pragma unroll
+    for (int t = 0; t < 4; t++) {
+      int o[3] = { 1, 1, 1 };
+      const int s1 = ((t >> 1) & 1) ? 1 : -1, s2 = (t & 1) ? 1 : -1;
+      o[o1] += s1; o[o2] += s2;
+      const long cn = cell_at(m, ii[o[0]], jj[o[1]], kk[o[2]]);
+      x[t] = rc.q[cn] - q0;
+      double gr[3]; rc.grad_ref(cn, gr);
+      x[4 + 2 * t] = gr[AX];
+      x[5 + 2 * t] = s1 * gr[o1] + s2 * gr[o2];
+    }
+    acc_edge<AX>(x, a);
+  }
+}
+
+template <bool CART>
+__global__ void __launch_bounds__(128, 3) recon_kernel(Mesh m, Slab sl, const double* __restrict__ W, double* __restrict__ pv,
                                                     double* __restrict__ chi_out, ReconPrm rp, int kA, long nthreads,
                                                     int* __restrict__ flag) {
   const long t = (long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -30,59 +93,38 @@ __global__ void __launch_bounds__(128) recon_kernel(Mesh m, Slab sl, const doubl
   const int ii[3] = { wrap(x.i - 1, m.ni), x.i, wrap(x.i + 1, m.ni) };
   const int jj[3] = { wrap(x.j - 1, m.nj), x.j, wrap(x.j + 1, m.nj) };
   const int kk[3] = { wrap(x.k - 1, m.nk), x.k, wrap(x.k + 1, m.nk) };
-  double J[9], Ji[9];
+  ReconCell<CART> rc{ m, W + (long)planeQ(v) * n, W + (long)planeG(v, 0) * n, W + (long)planeG(v, 1) * n, W + (long)planeG(v, 2) * n, {} };
   if (!CART) {
 #pragma unroll
-    for (int q = 0; q < 9; q++) { J[q] = m.met[(MET_J0 + q) * n + x.c]; Ji[q] = m.met[(MET_J0INV + q) * n + x.c]; }
+    for (int q = 0; q < 9; q++) rc.J[q] = m.met[(MET_J0 + q) * n + x.c];
   }
-  const double* q = W + (long)planeQ(v) * n;
-  const double* G0 = W + (long)planeG(v, 0) * n;
-  const double* G1 = W + (long)planeG(v, 1) * n;
-  const double* G2 = W + (long)planeG(v, 2) * n;
-  const double q0 = q[x.c];
-  double d[72];
-  // 18 neighbours: faces m = 2*axis + (0:+,1:-); edges e = 4*z0 + 2*(s1>0) + (s2>0)
+  const double q0 = rc.q[x.c];
+  double a[34], dface[6], la[3];
 #pragma unroll
-  for (int nb = 0; nb < 18; nb++) {
-    int o[3] = { 0, 0, 0 }; int z0 = -1;
-    if (nb < 6) { o[nb / 2] = (nb % 2 == 0) ? 1 : -1; }
-    else {
-      const int e = nb - 6; z0 = e / 4;
-      const int o1 = (z0 == 0) ? 1 : 0, o2 = (z0 == 2) ? 1 : 2;
-      o[o1] = ((e >> 1) & 1) ? 1 : -1; o[o2] = (e & 1) ? 1 : -1;
-    }
-    const long cn = cell_at(m, ii[o[0] + 1], jj[o[1] + 1], kk[o[2] + 1]);
-    d[nb] = q[cn] - q0;
-    const double g0 = G0[cn], g1 = G1[cn], g2 = G2[cn];
-    double gr[3];      // (grad Q)' = J0^T grad Q with the target cell's J0
-    if (CART) { gr[0] = m.h[0] * g0; gr[1] = m.h[1] * g1; gr[2] = m.h[2] * g2; }
-    else {
+  for (int b = 0; b < 34; b++) a[b] = 0.0;
+  recon_gather_axis<CART, 0>(rc, ii, jj, kk, q0, a, dface);
+  recon_gather_axis<CART, 1>(rc, ii, jj, kk, q0, a, dface);
+  recon_gather_axis<CART, 2>(rc, ii, jj, kk, q0, a, dface);
+  {   // line differences (Eq. 10): raw D, the factor h3' is folded into the coefficients
+    double Dl[4];
 #pragma unroll
-      for (int a = 0; a < 3; a++) gr[a] = J[a] * g0 + J[3 + a] * g1 + J[6 + a] * g2;
-    }
-    if (nb < 6) { d[18 + 3 * nb] = 2.0 * gr[0]; d[18 + 3 * nb + 1] = 2.0 * gr[1]; d[18 + 3 * nb + 2] = 2.0 * gr[2]; }
-    else {
-      const int e = nb - 6;
-      d[36 + 2 * e] = gr[z0];
-      d[36 + 2 * e + 1] = (o[0] * gr[0] + o[1] * gr[1] + o[2] * gr[2]) * 0.70710678118654752440;
-    }
+    for (int s = 0; s < 4; s++) Dl[s] = W[(long)planeD(v, s) * n + x.c];
+    la[0] = 0.25 * (Dl[0] + Dl[1] + Dl[2] + Dl[3]); acc_line<0>(Dl, a);
+#pragma unroll
+    for (int s = 0; s < 4; s++) Dl[s] = W[(long)planeD(v, 4 + s) * n + x.c];
+    la[1] = 0.25 * (Dl[0] + Dl[1] + Dl[2] + Dl[3]); acc_line<1>(Dl, a);
+#pragma unroll
+    for (int s = 0; s < 4; s++) Dl[s] = W[(long)planeD(v, 8 + s) * n + x.c];
+    la[2] = 0.25 * (Dl[0] + Dl[1] + Dl[2] + Dl[3]); acc_line<2>(Dl, a);
   }
-  double Dl[12];
-#pragma unroll
-  for (int s = 0; s < 12; s++) { Dl[s] = W[(long)planeD(v, s) * n + x.c]; d[60 + s] = 3.0 * Dl[s]; }
-  double a[34];
-  recon_Md(d, a);
   double chi = 1.0;
   if (rp.nonlinear) {
     // six linear polynomials (Eq. 15): normal slope = average difference, tangential = mean line difference
-    double la[3];
-#pragma unroll
-    for (int ax = 0; ax < 3; ax++) la[ax] = 0.25 * (Dl[4 * ax] + Dl[4 * ax + 1] + Dl[4 * ax + 2] + Dl[4 * ax + 3]);
     double wsum = 0.0, bw[3] = { 0, 0, 0 };
 #pragma unroll
     for (int mm = 0; mm < 6; mm++) {
       double b[3] = { la[0], la[1], la[2] };
-      b[mm / 2] = (mm % 2 == 0) ? d[mm] : -d[mm];
+      b[mm / 2] = (mm % 2 == 0) ? dface[mm] : -dface[mm];
       const double IS = b[0] * b[0] + b[1] * b[1] + b[2] * b[2];
       const double tt = IS + rp.eps, t2 = tt * tt;
       const double wb = (1.0 / 6.0) / (t2 * t2 * tt);               // d_m/(IS_m + eps)^5
@@ -105,21 +147,31 @@ __global__ void __launch_bounds__(128) recon_kernel(Mesh m, Slab sl, const doubl
   if (chi_out) chi_out[(long)v * n + x.c] = chi;
   // values and gradients at the 24 face Gauss points, back-transformed
   const long off = (long)slot_of(m, sl, x.k) * m.plane + x.ij;
-  double o[96];
-  recon_eval(a, o);
+  double Ji[9];
+  if (!CART) {
 #pragma unroll
-  for (int p = 0; p < 24; p++) {
-    double* dst = pv + (long)(p * 20) * sl.stride_pv + off;
-    dst[(long)v * sl.stride_pv] = q0 + o[4 * p];
-    double g[3];
-    if (CART) { g[0] = o[4 * p + 1] / m.h[0]; g[1] = o[4 * p + 2] / m.h[1]; g[2] = o[4 * p + 3] / m.h[2]; }
-    else {
-#pragma unroll
-      for (int r = 0; r < 3; r++) g[r] = Ji[r] * o[4 * p + 1] + Ji[3 + r] * o[4 * p + 2] + Ji[6 + r] * o[4 * p + 3];
-    }
-#pragma unroll
-    for (int r = 0; r < 3; r++) dst[(long)(5 + 3 * v + r) * sl.stride_pv] = g[r];
+    for (int q = 0; q < 9; q++) Ji[q] = m.met[(MET_J0INV + q) * n + x.c];
   }
+  const double ih[3] = { 1.0 / m.h[0], 1.0 / m.h[1], 1.0 / m.h[2] };
+  auto store_axis = [&](int ax, const double* o) {
+#pragma unroll
+    for (int l = 0; l < 8; l++) {
+      const int p = 8 * ax + l;            // = 4 * (2 ax + sgn) + 2a + b
+      double* dst = pv + (long)(p * 20) * sl.stride_pv + off;
+      dst[(long)v * sl.stride_pv] = q0 + o[4 * l];
+      double g[3];
+      if (CART) { g[0] = o[4 * l + 1] * ih[0]; g[1] = o[4 * l + 2] * ih[1]; g[2] = o[4 * l + 3] * ih[2]; }
+      else {
+#pragma unroll
+        for (int r = 0; r < 3; r++) g[r] = Ji[r] * o[4 * l + 1] + Ji[3 + r] * o[4 * l + 2] + Ji[6 + r] * o[4 * l + 3];
+      }
+#pragma unroll
+      for (int r = 0; r < 3; r++) dst[(long)(5 + 3 * v + r) * sl.stride_pv] = g[r];
+    }
+  };
+  { double o[32]; eval_axis<0>(a, o); store_axis(0, o); }
+  { double o[32]; eval_axis<1>(a, o); store_axis(1, o); }
+  { double o[32]; eval_axis<2>(a, o); store_axis(2, o); }
 }
 
 // ------------------------------------------------------------------------------------------------ flux
