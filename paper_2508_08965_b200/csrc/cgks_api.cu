@@ -108,8 +108,9 @@ static void collect_events(cgks_ctx* c) {
 static GasConst gas_const(const cgks_params& p) {
   GasConst g;
   g.K = (5.0 - 3.0 * p.gamma) / (p.gamma - 1.0);
+  g.inv_K3 = 1.0 / (g.K + 3.0);
   g.Pr_fix = (p.mu_ref > 0.0 && p.Pr != 1.0) ? (1.0 / p.Pr - 1.0) : 0.0;
-  g.mu_ref = p.mu_ref; g.omega = p.visc_omega; g.T_ref = p.T_ref; g.c1 = p.tau_c1; g.c2 = p.tau_c2;
+  g.mu_ref = p.mu_ref; g.omega = p.visc_omega; g.inv_T_ref = 1.0 / p.T_ref; g.c1 = p.tau_c1; g.c2 = p.tau_c2;
   return g;
 }
 
@@ -265,9 +266,12 @@ static void launch_flux(cgks_ctx* c, const Slab& sl, const double* Win, double d
   const long nt = (long)cnt * m.plane;
   dim3 grid((unsigned)((nt + TPB - 1) / TPB), 4);
   const GasConst gc = gas_const(c->prm);
-  { Timed t(c, KC_FLUX); flux_kernel<CART, 0><<<grid, TPB, 0, c->stream>>>(m, sl, Win, c->pv, c->fx, gc, dt, kA, nt, stage); }
-  { Timed t(c, KC_FLUX); flux_kernel<CART, 1><<<grid, TPB, 0, c->stream>>>(m, sl, Win, c->pv, c->fx, gc, dt, kA, nt, stage); }
-  { Timed t(c, KC_FLUX); flux_kernel<CART, 2><<<grid, TPB, 0, c->stream>>>(m, sl, Win, c->pv, c->fx, gc, dt, kA, nt, stage); }
+  const double idt = 1.0 / dt;
+#define CGKS_FLUX(AX) do { Timed t(c, KC_FLUX); \
+    if (stage == 2) flux_kernel<CART, AX, true><<<grid, TPB, 0, c->stream>>>(m, sl, Win, c->pv, c->fx, gc, dt, idt, kA, nt); \
+    else flux_kernel<CART, AX, false><<<grid, TPB, 0, c->stream>>>(m, sl, Win, c->pv, c->fx, gc, dt, idt, kA, nt); } while (0)
+  CGKS_FLUX(0); CGKS_FLUX(1); CGKS_FLUX(2);
+#undef CGKS_FLUX
 }
 
 template <bool CART>

@@ -11,6 +11,9 @@
 namespace cgks {
 
 struct ReconPrm { int nonlinear; double C, eps, inv_tanhC, gamma; };
+#ifndef FLUX_MINB
+#define FLUX_MINB 2
+#endif
 
 // ------------------------------------------------------------------------------------------------ reconstruction
 // Thread per (cell, variable).  PAPER.md:134-246 (Eq. 11-16), 250-300 (Eq. 17-19).
@@ -177,9 +180,9 @@ __global__ void __launch_bounds__(128, 3) recon_kernel(Mesh m, Slab sl, const do
 // ------------------------------------------------------------------------------------------------ flux
 // Thread per (cell, Gauss point q of the + face of AXIS); blockIdx.y = q.  PAPER.md:33-92, 330-352.
 // stage 2 stores only the time derivatives (reading T4).
-template <bool CART, int AXIS>
-__global__ void __launch_bounds__(128) flux_kernel(Mesh m, Slab sl, const double* __restrict__ W, const double* __restrict__ pv,
-                                                   double* __restrict__ fx, GasConst gc, double dt, int kA, long nthreads, int stage) {
+template <bool CART, int AXIS, bool STAGE2>
+__global__ void __launch_bounds__(128, FLUX_MINB) flux_kernel(Mesh m, Slab sl, const double* __restrict__ W, const double* __restrict__ pv,
+                                                   double* __restrict__ fx, GasConst gc, double dt, double idt, int kA, long nthreads) {
   const long t = (long)blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= nthreads) return;
   const int q = blockIdx.y;
@@ -258,11 +261,11 @@ __global__ void __launch_bounds__(128) flux_kernel(Mesh m, Slab sl, const double
     }
   }
   double out[6][5];      // Fn, Ft, VL, DL, VR, DR in the face frame
-  gks_flux_local(gc, dt, WL, SL, WR, SR, out[0], out[1], out[2], out[3], out[4], out[5]);
+  gks_flux_local<STAGE2>(gc, dt, idt, WL, SL, WR, SR, out[0], out[1], out[2], out[3], out[4], out[5]);
   double* dst = fx + (long)((4 * AXIS + q) * 30) * sl.stride_fx + offL;
 #pragma unroll
   for (int g = 0; g < 6; g++) {
-    if (stage == 2 && (g == 0 || g == 2 || g == 4)) continue;
+    if (STAGE2 && (g == 0 || g == 2 || g == 4)) continue;
     double o3[3];
     if (CART) {
       const int p0 = AXIS, p1 = (AXIS + 1) % 3, p2 = (AXIS + 2) % 3;
