@@ -38,6 +38,7 @@ struct cgks_ctx {
   double* fx = nullptr;
   unsigned long long* d_dt = nullptr;   // [1] bit pattern of the reduced dt
   int* d_flags = nullptr;               // [0..2] geometry, [3] non-physical state
+  int nsm = 148;                        // multiprocessors of the device
   int S = 0;                            // slab depth in k-planes; S == nk: whole mesh resident
   int slots_pv = 0, slots_fx = 0;
   long launches = 0;
@@ -114,17 +115,34 @@ static GasConst gas_const(const cgks_params& p) {
   return g;
 }
 
+static cudaError_t set_flux_smem() {
+  cudaError_t e = cudaSuccess;
+#define CGKS_ATTR(C, A, S2) if (e == cudaSuccess) e = cudaFuncSetAttribute(flux_kernel<C, A, S2>, cudaFuncAttributeMaxDynamicSharedMemorySize, FLUX_SMEM_BYTES)
+  CGKS_ATTR(true, 0, true); CGKS_ATTR(true, 1, true); CGKS_ATTR(true, 2, true);
+  CGKS_ATTR(true, 0, false); CGKS_ATTR(true, 1, false); CGKS_ATTR(true, 2, false);
+  CGKS_ATTR(false, 0, true); CGKS_ATTR(false, 1, true); CGKS_ATTR(false, 2, true);
+  CGKS_ATTR(false, 0, false); CGKS_ATTR(false, 1, false); CGKS_ATTR(false, 2, false);
+#undef CGKS_ATTR
+  return e;
+}
+
 // ---- create / destroy -------------------------------------------------------------------------------------------
 extern "C" int cgks_create(cgks_ctx** out, int ni, int nj, int nk, const double* d_nodes, const cgks_params* params,
                            void* ws, size_t ws_bytes, void* stream) {
   if (!out) return CGKS_EINVAL;
   *out = nullptr;
   if (ni < 4 || nj < 4 || nk < 4 || !d_nodes || !params || !ws) return CGKS_EINVAL;
+  if ((double)ni * nj * nk >= 2147483648.0 / 8.0) return CGKS_EINVAL;      // 32-bit cell and tile indices in the kernels
   if (params->geno_r != 2 || !(params->gamma > 1.0) || !(params->gamma < 5.0 / 3.0 + 1e-12)) return CGKS_EINVAL;
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return CGKS_ECUDA;
   cgks_ctx* c = new cgks_ctx();
   c->prm = *params; c->stream = (cudaStream_t)stream;
+  {
+    int dev = 0; cudaGetDevice(&dev);
+    if (cudaDeviceGetAttribute(&c->nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || c->nsm <= 0) c->nsm = 148;
+    if (set_flux_smem() != cudaSuccess) { delete c; return CGKS_ECUDA; }
+  }
   Mesh& m = c->mesh;
   m.ni = ni; m.nj = nj; m.nk = nk; m.plane = (long)ni * nj; m.n = m.plane * nk; m.cart = 0; m.met = nullptr;
   const long n = m.n;
@@ -264,12 +282,14 @@ template <bool CART>
 static void launch_flux(cgks_ctx* c, const Slab& sl, const double* Win, double dt, int kA, int cnt, int stage) {
   const Mesh& m = c->mesh;
   const long nt = (long)cnt * m.plane;
-  dim3 grid((unsigned)((nt + TPB - 1) / TPB), 4);
+  const long ntiles = 4 * ((nt + FLUX_TPB - 1) / FLUX_TPB);
+  const long maxb = (long)c->nsm * FLUX_MINB;
+  const unsigned grid = (unsigned)(ntiles < maxb ? ntiles : maxb);        // persistent blocks, FLUX_MINB per SM
   const GasConst gc = gas_const(c->prm);
   const double idt = 1.0 / dt;
 #define CGKS_FLUX(AX) do { Timed t(c, KC_FLUX); \
-    if (stage == 2) flux_kernel<CART, AX, true><<<grid, TPB, 0, c->stream>>>(m, sl, Win, c->pv, c->fx, gc, dt, idt, kA, nt); \
-    else flux_kernel<CART, AX, false><<<grid, TPB, 0, c->stream>>>(m, sl, Win, c->pv, c->fx, gc, dt, idt, kA, nt); } while (0)
+    if (stage == 2) flux_kernel<CART, AX, true><<<grid, FLUX_TPB, FLUX_SMEM_BYTES, c->stream>>>(m, sl, Win, c->pv, c->fx, gc, dt, idt, kA, nt); \
+    else flux_kernel<CART, AX, false><<<grid, FLUX_TPB, FLUX_SMEM_BYTES, c->stream>>>(m, sl, Win, c->pv, c->fx, gc, dt, idt, kA, nt); } while (0)
   CGKS_FLUX(0); CGKS_FLUX(1); CGKS_FLUX(2);
 #undef CGKS_FLUX
 }

@@ -35,12 +35,14 @@ __device__ __forceinline__ int wrap(int i, int n) { return i < 0 ? i + n : (i >=
 __device__ __forceinline__ int slot_of(const Mesh& m, const Slab& s, int k) { int t = k - s.kbase; return t < 0 ? t + m.nk : t; }
 
 struct CellIdx { int i, j, k; long ij; long c; };
-// thread t over `cnt` planes starting at plane kA (wrapped)
+// thread t over `cnt` planes starting at plane kA (wrapped).  32-bit index arithmetic: cgks_create rejects meshes with
+// 2^31 cells or more (far beyond 180 GB of state), and 64-bit integer division costs ~100 instructions on the SM.
 __device__ __forceinline__ CellIdx cell_of(const Mesh& m, long t, int kA) {
   CellIdx x;
-  int kk = (int)(t / m.plane); x.ij = t - (long)kk * m.plane;
-  x.j = (int)(x.ij / m.ni); x.i = (int)(x.ij - (long)x.j * m.ni);
-  x.k = kA + kk; if (x.k >= m.nk) x.k -= m.nk;
+  const unsigned tu = (unsigned)t, pl = (unsigned)m.plane, ni = (unsigned)m.ni;
+  const unsigned kk = tu / pl, ij = tu - kk * pl, j = ij / ni;
+  x.ij = ij; x.j = (int)j; x.i = (int)(ij - j * ni);
+  x.k = kA + (int)kk; if (x.k >= m.nk) x.k -= m.nk;
   x.c = (long)x.k * m.plane + x.ij;
   return x;
 }

@@ -35,16 +35,23 @@ struct Maxw {
   double P4[2][2];                       // q + r <= 1 used
 };
 
-__device__ __forceinline__ void maxw_init(Maxw& g, const double* Wc, const GasConst& gc) {
+// scalars of the Maxwellian of the conservative state Wc.  ONE division: with re = rho E - |m|^2/2 = rho (rho e),
+// r = 1/(rho re) gives 1/rho = re r and 1/re = rho r; lambda = (K+3) rho/(4 rho e) = (K+3) rho^2/(4 re).
+__device__ __forceinline__ void maxw_scalars(Maxw& g, const double* Wc, const GasConst& gc) {
   g.rho = Wc[0];
-  g.irho = 1.0 / Wc[0];
+  const double re = Wc[0] * Wc[4] - 0.5 * (Wc[1] * Wc[1] + Wc[2] * Wc[2] + Wc[3] * Wc[3]);     // rho * (rho e)
+  const double r = 1.0 / (Wc[0] * re);
+  g.irho = re * r;
+  const double ire = Wc[0] * r;
   g.U = Wc[1] * g.irho; g.V = Wc[2] * g.irho; g.W = Wc[3] * g.irho;
-  const double e = Wc[4] - 0.5 * (Wc[1] * g.U + Wc[2] * g.V + Wc[3] * g.W);      // rho e = p (K+3)/2
-  g.hil = 2.0 * e * g.irho * gc.inv_K3;
-  g.lam = 0.5 / g.hil;
+  g.hil = 2.0 * gc.inv_K3 * re * (g.irho * g.irho);          // 1/(2 lam) = 2 (rho e)/((K+3) rho) = p/rho
+  g.lam = 0.25 * (gc.K + 3.0) * (Wc[0] * Wc[0]) * ire;
   const double k3h = (gc.K + 3.0) * g.hil;
   g.s = g.U * g.U + g.V * g.V + g.W * g.W + k3h;
   g.c4 = 4.0 * g.lam * g.lam * gc.inv_K3;
+}
+
+__device__ __forceinline__ void maxw_tables(Maxw& g, const GasConst& gc) {
   double mv[6], mw[6];
   mv[0] = 1.0; mv[1] = g.V; mw[0] = 1.0; mw[1] = g.W;
 #pragma unroll
@@ -64,6 +71,14 @@ __device__ __forceinline__ void maxw_init(Maxw& g, const double* Wc, const GasCo
     for (int r = 0; r + q < 2; r++)
       g.P4[q][r] = mv[q + 4] * mw[r] + mv[q] * mw[r + 4] + x4 * g.P0[q][r]
                  + 2.0 * (mv[q + 2] * mw[r + 2] + x2 * (mv[q + 2] * mw[r] + mv[q] * mw[r + 2]));
+}
+
+// first two half-space moments (times rho) of a Maxwellian: SGN = +1 -> u > 0, -1 -> u < 0
+__device__ __forceinline__ void half_moments(const Maxw& g, double SGN, double& mh0, double& mh1) {
+  const double isl = sqrt(2.0 * g.hil), sl = g.lam * isl;                      // 1/sqrt(lam), sqrt(lam)
+  const double ex = 0.28209479177387814347 * exp(-g.lam * g.U * g.U) * isl;    // 1/2 e^{-lam U^2}/sqrt(pi lam)
+  mh0 = g.rho * (0.5 * erfc(-SGN * sl * g.U));
+  mh1 = g.U * mh0 + SGN * (g.rho * ex);
 }
 
 // <u^0..u^(N-1)> from the first two
@@ -171,18 +186,12 @@ struct Groups {        // moments of the groups of Eq. 5 that are shared between
 };
 
 // one side (SGN = +1: left state, u > 0; SGN = -1: right state, u < 0)
-template <int SGN>
-__device__ __forceinline__ void gks_side(const GasConst& gc, const double* Wc, const double (*S)[5], Groups& G,
-                                         double* dQs, double& p_side) {
-  Maxw g; maxw_init(g, Wc, gc);
-  p_side = g.rho * g.hil;
+__device__ __forceinline__ void gks_side(Maxw& g, double mh0, double mh1, const GasConst& gc, const double (*S)[5], Groups& G,
+                                         double* dQs) {
+  maxw_tables(g, gc);
   double mu[6], mh[7];
   mu[0] = 1.0; mu[1] = g.U; mom_recur<6>(mu, g.U, g.hil);
-  const double isl = sqrt(2.0 * g.hil), sl = g.lam * isl;                 // 1/sqrt(lam), sqrt(lam)
-  const double ex = 0.28209479177387814347 * exp(-g.lam * g.U * g.U) * isl;   // 1/2 e^{-lam U^2}/sqrt(pi lam)
-  // half-space moments, pre-scaled by rho
-  mh[0] = g.rho * (0.5 * erfc(-SGN * sl * g.U));
-  mh[1] = g.U * mh[0] + SGN * (g.rho * ex);
+  mh[0] = mh0; mh[1] = mh1;                      // half-space moments, pre-scaled by rho
   mom_recur<7>(mh, g.U, g.hil);
   add_plain<0>(g, mh, G.W0);
   add_plain<1>(g, mh, G.G4F);
@@ -240,11 +249,20 @@ __device__ __forceinline__ void gks_flux_local(const GasConst& gc, double dt, do
     G.W0[v] = 0; G.G4F[v] = 0; G.G5Q[v] = 0; G.G5F[v] = 0; G.G6Q[v] = 0; G.G6F[v] = 0;
     G.dW0[0][v] = 0; G.dW0[1][v] = 0; G.dW0[2][v] = 0;
   }
+  // scalars and half-space moments of both sides first: the two erfc/exp/sqrt/reciprocal chains are independent and
+  // overlap in the FP64 pipe; the tables and slopes of each side follow
   double pl, pr;
-  gks_side<+1>(gc, WL, SL, G, DL, pl);     // DL, DR hold the one-sided time derivatives for now
-  gks_side<-1>(gc, WR, SR, G, DR, pr);
+  {
+    Maxw gl, gr;
+    double hl0, hl1, hr0, hr1;
+    maxw_scalars(gl, WL, gc); maxw_scalars(gr, WR, gc);
+    half_moments(gl, 1.0, hl0, hl1); half_moments(gr, -1.0, hr0, hr1);
+    pl = gl.rho * gl.hil; pr = gr.rho * gr.hil;
+    gks_side(gl, hl0, hl1, gc, SL, G, DL);     // DL, DR hold the one-sided time derivatives for now
+    gks_side(gr, hr0, hr1, gc, SR, G, DR);
+  }
   // equilibrium state g0 and its slopes
-  Maxw g0; maxw_init(g0, G.W0, gc);
+  Maxw g0; maxw_scalars(g0, G.W0, gc); maxw_tables(g0, gc);
   double mu[7];
   mu[0] = g0.rho; mu[1] = g0.rho * g0.U; mom_recur<7>(mu, g0.U, g0.hil);     // full moments times rho0
   double G1F[5] = { 0, 0, 0, 0, 0 }, G2Q[5], G2F[5], G3F[5];
@@ -270,12 +288,11 @@ __device__ __forceinline__ void gks_flux_local(const GasConst& gc, double dt, do
   micro_slope(g0, h, a);
   { UPoly pa; make_upoly<0, 0>(pa, g0, a); apply_poly<3, 1, false>(pa.c, mu, G3F); }
   // collision time
-  const double p0 = g0.rho * g0.hil;
   double tau_phys = 0.0;
   if (gc.mu_ref > 0.0) {
     double visc = gc.mu_ref;
     if (gc.omega != 0.0) visc *= exp(gc.omega * log(g0.hil * gc.inv_T_ref));      // (T/T_ref)^omega, T = p/rho
-    tau_phys = visc / p0;
+    tau_phys = visc * (2.0 * g0.lam * g0.irho);                                    // mu / p0
   }
   const double dpr = fabs(pl - pr) / fabs(pl + pr);
   const double tau = tau_phys + gc.c1 * dt + gc.c2 * dpr * dt;
@@ -313,8 +330,9 @@ __device__ __forceinline__ void gks_flux_local(const GasConst& gc, double dt, do
     }
   }
   // one-sided interface values (reading F3): weight exp(-dt/tau0), tau0 = c2 |dp|/|sum p| dt
+  // (the weight is < 1e-300 when c2 dpr < 1/700: skipped there, which changes nothing above the 300th digit)
   double wgt = 0.0;
-  if (gc.c2 > 0.0 && dpr > 0.0) wgt = exp(-1.0 / (gc.c2 * dpr));
+  if (gc.c2 * dpr > 1.0 / 700.0) wgt = exp(-1.0 / (gc.c2 * dpr));
   const double om = 1.0 - wgt;
 #pragma unroll
   for (int v = 0; v < 5; v++) {

@@ -180,37 +180,100 @@ __global__ void __launch_bounds__(128, 3) recon_kernel(Mesh m, Slab sl, const do
 // ------------------------------------------------------------------------------------------------ flux
 // Thread per (cell, Gauss point q of the + face of AXIS); blockIdx.y = q.  PAPER.md:33-92, 330-352.
 // stage 2 stores only the time derivatives (reading T4).
+// Persistent blocks: each block walks over tiles of FLUX_TPB points (cells x Gauss point q of the + face of AXIS).
+// The 2 x 20 inputs of a point are staged by the owning thread itself with cp.async into its own column of a
+// double-buffered shared-memory tile, one tile ahead of the arithmetic, so the DRAM latency of the loads is hidden
+// behind the ~2000 FP64 instructions of the previous point (no block-level synchronisation is needed: a thread only
+// reads what it copied).
+__device__ __forceinline__ void cp_async8(double* smem_dst, const double* gsrc) {
+#ifdef FLUX_SYNC_COPY
+  *smem_dst = *gsrc; return;
+#endif
+  const unsigned sa = (unsigned)__cvta_generic_to_shared(smem_dst);
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(sa), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
+
+constexpr int FLUX_TPB = 128;
+constexpr int FLUX_SMEM_BYTES = 2 * 40 * FLUX_TPB * 8;
+
+struct FluxPoint { int q; long t; CellIdx x; int ir, jr, kr; long offL, offR; };
+
+template <int AXIS>
+__device__ __forceinline__ bool flux_point(const Mesh& m, const Slab& sl, long tile, long tiles_per_q, long ncells, int kA, FluxPoint& f) {
+  const unsigned tq = (unsigned)tile / (unsigned)tiles_per_q;
+  f.q = (int)tq;
+  f.t = (long)(((unsigned)tile - tq * (unsigned)tiles_per_q) * (unsigned)FLUX_TPB + threadIdx.x);
+  if (f.t >= ncells) return false;
+  f.x = cell_of(m, f.t, kA);
+  f.ir = f.x.i; f.jr = f.x.j; f.kr = f.x.k;
+  if (AXIS == 0) f.ir = wrap(f.x.i + 1, m.ni); else if (AXIS == 1) f.jr = wrap(f.x.j + 1, m.nj); else f.kr = wrap(f.x.k + 1, m.nk);
+  f.offL = (long)slot_of(m, sl, f.x.k) * m.plane + f.x.ij;
+  f.offR = (long)slot_of(m, sl, f.kr) * m.plane + (long)f.jr * m.ni + f.ir;
+  return true;
+}
+
 template <bool CART, int AXIS, bool STAGE2>
-__global__ void __launch_bounds__(128, FLUX_MINB) flux_kernel(Mesh m, Slab sl, const double* __restrict__ W, const double* __restrict__ pv,
-                                                   double* __restrict__ fx, GasConst gc, double dt, double idt, int kA, long nthreads) {
-  const long t = (long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (t >= nthreads) return;
-  const int q = blockIdx.y;
-  const CellIdx x = cell_of(m, t, kA);
-  // right cell
-  int ir = x.i, jr = x.j, kr = x.k;
-  if (AXIS == 0) ir = wrap(x.i + 1, m.ni); else if (AXIS == 1) jr = wrap(x.j + 1, m.nj); else kr = wrap(x.k + 1, m.nk);
-  const long offL = (long)slot_of(m, sl, x.k) * m.plane + x.ij;
-  const long offR = (long)slot_of(m, sl, kr) * m.plane + (long)jr * m.ni + ir;
-  const double* pL = pv + (long)((4 * (2 * AXIS) + q) * 20) * sl.stride_pv + offL;
-  const double* pR = pv + (long)((4 * (2 * AXIS + 1) + q) * 20) * sl.stride_pv + offR;
+__global__ void __launch_bounds__(FLUX_TPB, FLUX_MINB) flux_kernel(Mesh m, Slab sl, const double* __restrict__ W, const double* __restrict__ pv,
+                                                   double* __restrict__ fx, GasConst gc, double dt, double idt, int kA, long ncells) {
+  extern __shared__ double smf[];                     // [2][40][FLUX_TPB]
+  const long tiles_per_q = (ncells + FLUX_TPB - 1) / FLUX_TPB;
+  const long ntiles = 4 * tiles_per_q;
+  // returns whether this thread has a point in `tile`; its q and left offset are carried to the compute phase
+  auto issue = [&](long tile, int buf, int& q_out, long& offL_out, long& c_out) -> bool {
+    FluxPoint f;
+    const bool act = tile < ntiles && flux_point<AXIS>(m, sl, tile, tiles_per_q, ncells, kA, f);
+    if (act) {
+      const double* pL = pv + f.offL;
+      const double* pR = pv + f.offR;
+      const long planeL = (long)((4 * (2 * AXIS) + f.q) * 20), planeR = (long)((4 * (2 * AXIS + 1) + f.q) * 20);
+      double* dstL = smf + (long)(buf * 40) * FLUX_TPB + threadIdx.x;
+#pragma unroll
+      for (int c = 0; c < 20; c++) cp_async8(dstL + c * FLUX_TPB, pL + (planeL + c) * sl.stride_pv);
+#pragma unroll
+      for (int c = 0; c < 20; c++) cp_async8(dstL + (20 + c) * FLUX_TPB, pR + (planeR + c) * sl.stride_pv);
+      q_out = f.q; offL_out = f.offL; c_out = f.x.c;
+    }
+    cp_async_commit();
+    return act;
+  };
+  int buf = 0, q = 0, qn = 0;
+  long offL = 0, offLn = 0, cL = 0, cLn = 0;
+  bool active = issue(blockIdx.x, 0, q, offL, cL), activen = false;
+#pragma unroll 1
+  for (long tile = blockIdx.x; tile < ntiles; tile += gridDim.x, buf ^= 1, q = qn, offL = offLn, cL = cLn, active = activen) {
+  cp_async_wait<0>();
+  const double* sL = smf + (long)(buf * 40) * FLUX_TPB + threadIdx.x;
   double WLg[5], WRg[5], gL[15], gR[15];
 #pragma unroll
-  for (int c = 0; c < 5; c++) { WLg[c] = pL[(long)c * sl.stride_pv]; WRg[c] = pR[(long)c * sl.stride_pv]; }
+  for (int c = 0; c < 5; c++) { WLg[c] = sL[c * FLUX_TPB]; WRg[c] = sL[(20 + c) * FLUX_TPB]; }
 #pragma unroll
-  for (int c = 0; c < 15; c++) { gL[c] = pL[(long)(5 + c) * sl.stride_pv]; gR[c] = pR[(long)(5 + c) * sl.stride_pv]; }
+  for (int c = 0; c < 15; c++) { gL[c] = sL[(5 + c) * FLUX_TPB]; gR[c] = sL[(25 + c) * FLUX_TPB]; }
+  activen = issue(tile + gridDim.x, buf ^ 1, qn, offLn, cLn);      // next tile's inputs stream in while this point is computed
+  if (!active) continue;
+#ifdef FLUX_DEBUG_ECHO
+  {
+    double* dste = fx + (long)((4 * AXIS + q) * 30) * sl.stride_fx + offL;
+    for (int c = 0; c < 5; c++) { dste[(long)c * sl.stride_fx] = WLg[c]; dste[(long)(5 + c) * sl.stride_fx] = WRg[c]; }
+    for (int c = 0; c < 15; c++) dste[(long)(10 + c) * sl.stride_fx] = gR[c];
+    for (int c = 0; c < 5; c++) dste[(long)(25 + c) * sl.stride_fx] = gL[c];
+    continue;
+  }
+#endif
   // positivity (reading R9, point-wise): a non-physical reconstructed state falls back to the cell average
   {
-    const double eL = WLg[4] - 0.5 * (WLg[1] * WLg[1] + WLg[2] * WLg[2] + WLg[3] * WLg[3]) / WLg[0];
+    const double eL = WLg[0] * WLg[4] - 0.5 * (WLg[1] * WLg[1] + WLg[2] * WLg[2] + WLg[3] * WLg[3]);    // rho * (rho e)
     if (!(WLg[0] > 0.0) || !(eL > 0.0)) {
 #pragma unroll
-      for (int c = 0; c < 5; c++) WLg[c] = W[(long)c * m.n + x.c];
+      for (int c = 0; c < 5; c++) WLg[c] = W[(long)c * m.n + cL];
 #pragma unroll
       for (int c = 0; c < 15; c++) gL[c] = 0.0;
     }
-    const double eR = WRg[4] - 0.5 * (WRg[1] * WRg[1] + WRg[2] * WRg[2] + WRg[3] * WRg[3]) / WRg[0];
+    const double eR = WRg[0] * WRg[4] - 0.5 * (WRg[1] * WRg[1] + WRg[2] * WRg[2] + WRg[3] * WRg[3]);
     if (!(WRg[0] > 0.0) || !(eR > 0.0)) {
-      const long cr = cell_at(m, ir, jr, kr);
+      FluxPoint fp; flux_point<AXIS>(m, sl, tile, tiles_per_q, ncells, kA, fp);
+      const long cr = cell_at(m, fp.ir, fp.jr, fp.kr);
 #pragma unroll
       for (int c = 0; c < 5; c++) WRg[c] = W[(long)c * m.n + cr];
 #pragma unroll
@@ -235,7 +298,7 @@ __global__ void __launch_bounds__(128, FLUX_MINB) flux_kernel(Mesh m, Slab sl, c
   } else {
     double A[3];
 #pragma unroll
-    for (int r = 0; r < 3; r++) { A[r] = m.met[(MET_AREA + 3 * AXIS + r) * m.n + x.c]; fr[1][r] = m.met[(MET_TAN + 3 * AXIS + r) * m.n + x.c]; }
+    for (int r = 0; r < 3; r++) { A[r] = m.met[(MET_AREA + 3 * AXIS + r) * m.n + cL]; fr[1][r] = m.met[(MET_TAN + 3 * AXIS + r) * m.n + cL]; }
     const double S = sqrt(A[0] * A[0] + A[1] * A[1] + A[2] * A[2]);
 #pragma unroll
     for (int r = 0; r < 3; r++) fr[0][r] = A[r] / S;
@@ -280,6 +343,7 @@ __global__ void __launch_bounds__(128, FLUX_MINB) flux_kernel(Mesh m, Slab sl, c
     dst[(long)(5 * g + 3) * sl.stride_fx] = o3[2];
     dst[(long)(5 * g + 4) * sl.stride_fx] = out[g][4];
   }
+  }   // tile loop
 }
 
 // ------------------------------------------------------------------------------------------------ update
