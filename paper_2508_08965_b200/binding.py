@@ -55,6 +55,7 @@ def lib():
         L.cgks_get_chi.argtypes = [_vp, _vp]
         L.cgks_debug_stage.argtypes = [_vp, C.c_double, _vp, _vp]
         L.cgks_fp64_peak.argtypes = [_vp, C.POINTER(C.c_double)]
+        L.cgks_debug_math.argtypes = [C.c_int, C.c_long, _vp, _vp, _vp]
         L.cgks_destroy.argtypes = [_vp]
         L.cgks_last_error.argtypes = [_vp]; L.cgks_last_error.restype = C.c_char_p
         L.cgks_version.restype = C.c_char_p
@@ -84,6 +85,18 @@ def fp64_peak_tflops(device="cuda:0"):
     if rc:
         raise CgksError(rc, "cgks_fp64_peak")
     return out.value
+
+
+def debug_math(which, x, device="cuda:0"):
+    """Test tap cgks_debug_math: 0 1/x, 1 1/sqrt(x), 2 exp(x), 3 erfc(x), 4 exp(-x^2); x a float64 array."""
+    xin = _dev(x, torch.device(device)).reshape(-1)
+    out = torch.empty_like(xin)
+    with torch.cuda.device(xin.device):
+        st = torch.cuda.current_stream()
+        rc = lib().cgks_debug_math(int(which), xin.numel(), _ptr(xin), _ptr(out), _vp(st.cuda_stream))
+    if rc:
+        raise CgksError(rc, "cgks_debug_math")
+    return out.cpu().numpy()
 
 
 def _dev(a, device):

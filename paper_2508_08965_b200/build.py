@@ -7,7 +7,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libcgks.so")
 SOURCES = ["cgks_api.cu"]
-HEADERS = ["cgks_common.cuh", "kernels_setup.cuh", "kernels_stage.cuh", "gks_flux.cuh", "recon_gen.cuh"]
+HEADERS = ["cgks_common.cuh", "kernels_setup.cuh", "kernels_stage.cuh", "gks_flux.cuh", "fastmath64.cuh", "recon_gen.cuh", "math_gen.cuh"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared"]
 
@@ -19,6 +19,9 @@ def _newer(a, b):
 def generate(force=False):
     gen = os.path.join(CSRC, "gen_recon.py"); out = os.path.join(CSRC, "recon_gen.cuh")
     if force or not os.path.exists(out) or _newer(gen, out):
+        subprocess.check_call([sys.executable, gen])
+    gen = os.path.join(CSRC, "gen_math.py"); out2 = os.path.join(CSRC, "math_gen.cuh")
+    if force or not os.path.exists(out2) or _newer(gen, out2):
         subprocess.check_call([sys.executable, gen])
     return out
 

@@ -436,3 +436,23 @@ extern "C" int cgks_run_host(cgks_ctx* c, const double* hQ, const double* hG, co
   if (oD) CK(cudaMemcpyAsync(oD, Wc + 20 * n, (size_t)60 * n * 8, cudaMemcpyDeviceToHost, c->stream));
   return cgks_status(c);
 }
+
+// ---- test tap: special functions of the flux kernel ------------------------------------------------------------------
+__global__ void debug_math_kernel(int which, long n, const double* __restrict__ in, double* __restrict__ out) {
+  const long t = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= n) return;
+  const double x = in[t];
+  double r = 0.0, e = 0.0;
+  if (which == 0) r = drcp(x);
+  else if (which == 1) r = drsqrt(x);
+  else if (which == 2) r = dexp(x);
+  else { derfc_exp(x, r, e); if (which == 4) r = e; }
+  out[t] = r;
+}
+
+extern "C" int cgks_debug_math(int which, long n, const double* d_in, double* d_out, void* stream) {
+  if (which < 0 || which > 4 || n < 0 || !d_in || !d_out) return CGKS_EINVAL;
+  if (n == 0) return CGKS_OK;
+  debug_math_kernel<<<(unsigned)((n + 255) / 256), 256, 0, (cudaStream_t)stream>>>(which, n, d_in, d_out);
+  return cudaGetLastError() == cudaSuccess ? CGKS_OK : CGKS_ECUDA;
+}

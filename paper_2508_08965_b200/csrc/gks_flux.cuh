@@ -14,6 +14,7 @@
 // serves the compatibility condition (full u-moments), the conserved moments (shift 0) and the flux moments (shift 1).
 #pragma once
 #include <math.h>
+#include "fastmath64.cuh"
 
 namespace cgks {
 
@@ -40,7 +41,7 @@ struct Maxw {
 __device__ __forceinline__ void maxw_scalars(Maxw& g, const double* Wc, const GasConst& gc) {
   g.rho = Wc[0];
   const double re = Wc[0] * Wc[4] - 0.5 * (Wc[1] * Wc[1] + Wc[2] * Wc[2] + Wc[3] * Wc[3]);     // rho * (rho e)
-  const double r = 1.0 / (Wc[0] * re);
+  const double r = drcp(Wc[0] * re);
   g.irho = re * r;
   const double ire = Wc[0] * r;
   g.U = Wc[1] * g.irho; g.V = Wc[2] * g.irho; g.W = Wc[3] * g.irho;
@@ -75,9 +76,11 @@ __device__ __forceinline__ void maxw_tables(Maxw& g, const GasConst& gc) {
 
 // first two half-space moments (times rho) of a Maxwellian: SGN = +1 -> u > 0, -1 -> u < 0
 __device__ __forceinline__ void half_moments(const Maxw& g, double SGN, double& mh0, double& mh1) {
-  const double isl = sqrt(2.0 * g.hil), sl = g.lam * isl;                      // 1/sqrt(lam), sqrt(lam)
-  const double ex = 0.28209479177387814347 * exp(-g.lam * g.U * g.U) * isl;    // 1/2 e^{-lam U^2}/sqrt(pi lam)
-  mh0 = g.rho * (0.5 * erfc(-SGN * sl * g.U));
+  const double sl = drsqrt(2.0 * g.hil), isl = 2.0 * g.hil * sl;               // sqrt(lam), 1/sqrt(lam)
+  double ec, E;
+  derfc_exp(-SGN * (sl * g.U), ec, E);                                         // erfc(-+ sqrt(lam) U), exp(-lam U^2)
+  const double ex = 0.28209479177387814347 * E * isl;                          // 1/2 e^{-lam U^2}/sqrt(pi lam)
+  mh0 = g.rho * (0.5 * ec);
   mh1 = g.U * mh0 + SGN * (g.rho * ex);
 }
 
@@ -291,17 +294,17 @@ __device__ __forceinline__ void gks_flux_local(const GasConst& gc, double dt, do
   double tau_phys = 0.0;
   if (gc.mu_ref > 0.0) {
     double visc = gc.mu_ref;
-    if (gc.omega != 0.0) visc *= exp(gc.omega * log(g0.hil * gc.inv_T_ref));      // (T/T_ref)^omega, T = p/rho
+    if (gc.omega != 0.0) visc *= dexp(gc.omega * log(g0.hil * gc.inv_T_ref));      // (T/T_ref)^omega, T = p/rho
     tau_phys = visc * (2.0 * g0.lam * g0.irho);                                    // mu / p0
   }
-  const double dpr = fabs(pl - pr) / fabs(pl + pr);
+  const double dpr = ddiv(fabs(pl - pr), fabs(pl + pr));
   const double tau = tau_phys + gc.c1 * dt + gc.c2 * dpr * dt;
   double c1[6], c2[6];
   if (tau == 0.0) {     // reading T2: f = g0 (1 + Abar t)
     c1[0] = dt; c1[1] = 0; c1[2] = 0.5 * dt * dt; c1[3] = c1[4] = c1[5] = 0;
     c2[0] = 0.5 * dt; c2[1] = 0; c2[2] = 0.125 * dt * dt; c2[3] = c2[4] = c2[5] = 0;
   } else {
-    const double E2 = exp(-0.5 * dt / tau), E1 = E2 * E2;
+    const double E2 = dexp(-0.5 * dt * drcp(tau)), E1 = E2 * E2;
     time_coef(dt, tau, E1, c1); time_coef(0.5 * dt, tau, E2, c2);
   }
   // f^n = (4 fbar(dt/2) - fbar(dt))/dt,  f_t^n = 4 (fbar(dt) - 2 fbar(dt/2))/dt^2
@@ -332,7 +335,7 @@ __device__ __forceinline__ void gks_flux_local(const GasConst& gc, double dt, do
   // one-sided interface values (reading F3): weight exp(-dt/tau0), tau0 = c2 |dp|/|sum p| dt
   // (the weight is < 1e-300 when c2 dpr < 1/700: skipped there, which changes nothing above the 300th digit)
   double wgt = 0.0;
-  if (gc.c2 * dpr > 1.0 / 700.0) wgt = exp(-1.0 / (gc.c2 * dpr));
+  if (gc.c2 * dpr > 1.0 / 700.0) wgt = dexp(-drcp(gc.c2 * dpr));
   const double om = 1.0 - wgt;
 #pragma unroll
   for (int v = 0; v < 5; v++) {

@@ -196,7 +196,10 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
 
 constexpr int FLUX_TPB = 128;
-constexpr int FLUX_SMEM_BYTES = 2 * 40 * FLUX_TPB * 8;
+#ifndef FLUX_NBUF
+#define FLUX_NBUF 1
+#endif
+constexpr int FLUX_SMEM_BYTES = FLUX_NBUF * 40 * FLUX_TPB * 8;
 
 struct FluxPoint { int q; long t; CellIdx x; int ir, jr, kr; long offL, offR; };
 
@@ -242,7 +245,7 @@ __global__ void __launch_bounds__(FLUX_TPB, FLUX_MINB) flux_kernel(Mesh m, Slab 
   long offL = 0, offLn = 0, cL = 0, cLn = 0;
   bool active = issue(blockIdx.x, 0, q, offL, cL), activen = false;
 #pragma unroll 1
-  for (long tile = blockIdx.x; tile < ntiles; tile += gridDim.x, buf ^= 1, q = qn, offL = offLn, cL = cLn, active = activen) {
+  for (long tile = blockIdx.x; tile < ntiles; tile += gridDim.x, buf ^= (FLUX_NBUF - 1), q = qn, offL = offLn, cL = cLn, active = activen) {
   cp_async_wait<0>();
   const double* sL = smf + (long)(buf * 40) * FLUX_TPB + threadIdx.x;
   double WLg[5], WRg[5], gL[15], gR[15];
@@ -250,7 +253,7 @@ __global__ void __launch_bounds__(FLUX_TPB, FLUX_MINB) flux_kernel(Mesh m, Slab 
   for (int c = 0; c < 5; c++) { WLg[c] = sL[c * FLUX_TPB]; WRg[c] = sL[(20 + c) * FLUX_TPB]; }
 #pragma unroll
   for (int c = 0; c < 15; c++) { gL[c] = sL[(5 + c) * FLUX_TPB]; gR[c] = sL[(25 + c) * FLUX_TPB]; }
-  activen = issue(tile + gridDim.x, buf ^ 1, qn, offLn, cLn);      // next tile's inputs stream in while this point is computed
+  activen = issue(tile + gridDim.x, buf ^ (FLUX_NBUF - 1), qn, offLn, cLn);      // next tile's inputs stream in while this point is computed
   if (!active) continue;
 #ifdef FLUX_DEBUG_ECHO
   {

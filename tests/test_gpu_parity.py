@@ -166,3 +166,32 @@ def test_chi_matches_oracle():
     chi_g = s.chi().cpu().numpy()
     assert chi_g.min() < 1e-3 and (chi_g[0] < 0.99).mean() > 0.05
     s.close()
+
+
+def test_special_functions_of_the_flux_kernel():
+    """csrc/fastmath64.cuh (branch-free reciprocal, rsqrt, exp, erfc with its exp(-x^2)) against mpmath (40 digits) on
+    sampled arguments: relative error <= 2e-15; dense checks against numpy/scipy, whose own erfc and exp(-x*x) carry
+    the rounding error of x*x (up to 6e-14 at |x| = 26), with correspondingly looser bounds."""
+    import mpmath as mp
+    from scipy import special
+    from paper_2508_08965_b200 import binding
+    rng = np.random.default_rng(7)
+    x = np.concatenate([10.0 ** rng.uniform(-12, 12, 20000), rng.uniform(0.5, 2.0, 20000)])
+    np.testing.assert_allclose(binding.debug_math(0, x), 1.0 / x, rtol=4e-16)
+    np.testing.assert_allclose(binding.debug_math(1, x), 1.0 / np.sqrt(x), rtol=6e-16)
+    xe = np.concatenate([rng.uniform(-700, 10, 20000), rng.uniform(-1, 1, 20000)])
+    np.testing.assert_allclose(binding.debug_math(2, xe), np.exp(xe), rtol=1e-15)
+    xu = np.array([-745.0, -760.0, -800.0, -1e5, -1e300])
+    assert np.all(binding.debug_math(2, xu) <= 1e-323 * 2)          # underflows gradually to 0, never garbage
+    xs = np.concatenate([rng.uniform(-6, 6, 40000), [0.0, 1e-300, -1e-300, 30.0, -30.0]])
+    np.testing.assert_allclose(binding.debug_math(3, xs), special.erfc(xs), rtol=5e-14, atol=1e-300)
+    np.testing.assert_allclose(binding.debug_math(4, xs), np.exp(-xs * xs), rtol=1e-14, atol=1e-300)
+    mp.mp.dps = 40
+    xm = np.concatenate([rng.uniform(-6, 6, 600), rng.uniform(6, 26, 200), rng.uniform(-1e-3, 1e-3, 100)])
+    xa = -np.abs(xm) * 25
+    ge = binding.debug_math(3, xm); gq = binding.debug_math(4, xm); gx = binding.debug_math(2, xa)
+    for a, b, c, d, e in zip(xm, ge, gq, gx, xa):
+        am = mp.mpf(float(a))
+        assert abs(mp.mpf(float(b)) / mp.erfc(am) - 1) < 2e-15, a
+        assert abs(mp.mpf(float(c)) / mp.exp(-am * am) - 1) < 2e-15, a
+        assert abs(mp.mpf(float(d)) / mp.exp(mp.mpf(float(e))) - 1) < 2e-15, e
