@@ -23,8 +23,17 @@ sys.path.insert(0, ROOT)
 
 METRIC = "cell-updates/s per S2O4 step (fp64)"
 UNIT = "cell-updates/s"
-# algorithmic fp64 flops of the dominant kernel (gas-kinetic flux) per face Gauss point: DESIGN.md section 7
-FLUX_FLOPS_PER_POINT = 4808.0
+# Dominant kernel = gas-kinetic flux (flux_kernel).  Algorithmic fp64 flops per face Gauss point of the formulation as
+# built (FMA = 2, add/mul = 1, including the Newton / polynomial arithmetic of its own reciprocal, rsqrt, exp and erfc in
+# csrc/fastmath64.cuh): stage 1 computes F, F_t, Q, Q_t and both one-sided values, stage 2 only the time derivatives.
+# Counted by ncu's executed-FP64-op counters on the committed capture profiles/r01d_kernels_128.md (1110.6 DFMA +
+# 645.1 DMUL + 226.4 DADD per point in stage 1; 1044.9 + 613.0 + 220.4 in stage 2); DESIGN.md section 7.
+FLUX_FLOPS_STAGE1 = 3092.7
+FLUX_FLOPS_STAGE2 = 2923.2
+# DRAM bytes per point of the same capture (dram__bytes_read + write per launch / points): the algorithmic bytes are
+# 40 inputs + 30 (stage 1) or 15 (stage 2) outputs of 8 B = 560 / 440 B
+FLUX_TRAFFIC_STAGE1 = 555.5
+FLUX_TRAFFIC_STAGE2 = 437.3
 FP64_PEAK_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12      # SMs x FP64 FMA lanes x 2 x max SM clock = 37.2
 
 
@@ -215,14 +224,19 @@ def run_ours(args):
     if fnl > 0:
         # every flux launch covers 4 Gauss points of one face direction of its cells; summed over the launches of the
         # timed region the points are 12 per cell per stage (+ the recomputed halo plane of each slab, counted in fnl)
-        pts_per_step = 2 * 12 * cells * slab_overhead(solver, n)
-        flops = FLUX_FLOPS_PER_POINT * pts_per_step * args.steps
+        pts_per_stage = 12 * cells * slab_overhead(solver, n)
+        flops = (FLUX_FLOPS_STAGE1 + FLUX_FLOPS_STAGE2) * pts_per_stage * args.steps
         ach = flops / (fms * 1e-3) / 1e12
+        pts_per_launch = 2 * pts_per_stage * args.steps / fnl
         roof = {"bound": "alu", "kernel": "flux_kernel", "achieved": ach, "peak": FP64_PEAK_NOMINAL_TFLOPS, "unit": "TFLOP/s",
-                "frac": ach / FP64_PEAK_NOMINAL_TFLOPS, "traffic": None,
+                "frac": ach / FP64_PEAK_NOMINAL_TFLOPS,
+                "traffic": 0.5 * (FLUX_TRAFFIC_STAGE1 + FLUX_TRAFFIC_STAGE2) * pts_per_launch,
+                "traffic_note": "bytes per average launch = ncu dram bytes per point (profiles/r01d_kernels_128.md) x points per launch; "
+                                "algorithmic bytes per point 560 (stage 1) / 440 (stage 2)",
                 "peak_source": "derived: 148 SMs x 64 FP64 FMA lanes x 2 x 1.965 GHz (DESIGN.md section 7); "
                                "MEASURED_PEAKS.json has no FP64 entry",
-                "peak_dfma_microbench": peak_meas, "avg_launch_ms": fms / fnl, "launches": fnl,
+                "peak_dfma_microbench": peak_meas, "frac_of_dfma_microbench": (ach / peak_meas) if peak_meas else None,
+                "avg_launch_ms": fms / fnl, "launches": fnl,
                 "share_of_step": fms / (ms if ms > 0 else 1.0),
                 "kernel_ms_per_step": {k: v[0] / args.steps for k, v in kms.items()}}
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
