@@ -1,0 +1,76 @@
+"""Host-side checks of the C ABI (no GPU needed): the library loads, exports every function include/cgks.h declares,
+and its pure host entry points behave as documented."""
+import ctypes as C
+import os
+import re
+
+import pytest
+
+from paper_2508_08965_b200 import binding, build
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    build.build()
+    return binding.lib()
+
+
+def declared_functions():
+    src = open(os.path.join(ROOT, "include", "cgks.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(cgks_[a-z0-9_]+)\s*\(", src)))
+
+
+def test_every_declared_symbol_is_exported(lib):
+    names = declared_functions()
+    assert {"cgks_create", "cgks_set_state", "cgks_compute_dt", "cgks_step", "cgks_get_state", "cgks_destroy",
+            "cgks_workspace_bytes", "cgks_run_host", "cgks_status"} <= set(names)
+    for nm in names:
+        assert hasattr(lib, nm), nm
+    raw = C.CDLL(binding.LIB_PATH)
+    for nm in names:
+        getattr(raw, nm)          # raises AttributeError if the symbol is missing
+
+
+def test_version_and_workspace_sizes(lib):
+    assert b"sm_100a" in lib.cgks_version()
+    small = binding.workspace_bytes(16, 16, 16)
+    fixed = (3 * 80 + 5 + 37) * 16 ** 3 * 8
+    assert small >= fixed + (480 + 360) * 16 ** 3 * 8          # whole mesh resident
+    big = binding.workspace_bytes(384, 384, 384)
+    assert 100e9 < big < 185e9                                  # three state buffers, metrics, ~48 GB of slab buffers
+    capped = binding.workspace_bytes(384, 384, 384, int(150e9))
+    assert capped <= 150e9 + 4096 and capped < big
+    with pytest.raises(binding.CgksError) as e:
+        binding.workspace_bytes(3, 16, 16)
+    assert e.value.code == binding.CGKS_EINVAL
+
+
+def test_no_cpu_fallback(lib):
+    """Without a CUDA device every compute entry point refuses: the product path never routes through the CPU."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a CUDA device is present")
+    h = C.c_void_p(None)
+    prm = binding.make_params()
+    dummy = (C.c_double * 8)()
+    rc = lib.cgks_create(C.byref(h), 8, 8, 8, C.cast(dummy, C.c_void_p), C.byref(prm), C.cast(dummy, C.c_void_p), 64, None)
+    assert rc == binding.CGKS_ECUDA and not h.value
+    with pytest.raises(RuntimeError):
+        binding.Solver(__import__("numpy").zeros((3, 9, 9, 9)), prm)
+    assert lib.cgks_step(None, 0.1) == binding.CGKS_EINVAL
+    assert lib.cgks_destroy(None) == binding.CGKS_EINVAL
+    assert lib.cgks_last_error(None) == b"null context"
+
+
+def test_product_path_does_not_import_the_oracle():
+    import subprocess
+    import sys
+    code = ("import sys; import paper_2508_08965_b200.binding, paper_2508_08965_b200.inputs, paper_2508_08965_b200.build; "
+            "bad = [m for m in sys.modules if m == 'oracle' or m.startswith('oracle.')]; sys.exit(1 if bad else 0)")
+    assert subprocess.run([sys.executable, "-c", code], cwd=ROOT).returncode == 0
+    for fn in os.listdir(os.path.join(ROOT, "paper_2508_08965_b200", "csrc")):
+        txt = open(os.path.join(ROOT, "paper_2508_08965_b200", "csrc", fn), errors="ignore").read()
+        assert "cgks_ref" not in txt and "oracle/" not in txt.replace("oracle/)", ""), fn

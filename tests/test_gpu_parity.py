@@ -195,3 +195,75 @@ def test_special_functions_of_the_flux_kernel():
         assert abs(mp.mpf(float(b)) / mp.erfc(am) - 1) < 2e-15, a
         assert abs(mp.mpf(float(c)) / mp.exp(-am * am) - 1) < 2e-15, a
         assert abs(mp.mpf(float(d)) / mp.exp(mp.mpf(float(e))) - 1) < 2e-15, e
+
+
+def _block(t, lo, size):
+    """Periodic sub-block [lo, lo+size)^3 of a (..., n, n, n) torch tensor (wraps around), as numpy."""
+    import torch
+    n = t.shape[-1]
+    idx = [torch.arange(l, l + size, device=t.device) % n for l in lo]      # lo = (k0, j0, i0)
+    return t.index_select(-3, idx[0]).index_select(-2, idx[1]).index_select(-1, idx[2]).cpu().numpy()
+
+
+@pytest.mark.parametrize("n,nblocks", [(384, 6), (96, 4)])
+def test_full_size_sampled_blocks(n, nblocks):
+    """BASELINE.json config 5 at its full size (384^3, the configuration bench.py times: slab pipeline, Cartesian
+    kernels), one S2O4 step, checked on sampled 16^3 blocks the oracle can compute on their own: a cell's new state
+    depends on cell averages within index distance 6 (bootstrap 2 + two stages of 2), so the oracle run on the periodic
+    28^3 block around a sample reproduces the inner 16^3 exactly, whatever happens at the block's own (wrong) periodic
+    seam.  Blocks are seeded, and include the periodic seam of the full mesh and a slab boundary of the pipeline.
+    The 96^3 case runs the same check with a workspace that forces a slab depth of 12."""
+    import torch
+    from oracle import ref
+    from paper_2508_08965_b200 import binding
+    dev = torch.device("cuda", 0)
+    free, _ = torch.cuda.mem_get_info(dev)
+    need = (3 * 80 + 5 + 480 + 360) * n ** 3 * 8
+    if n == 384 and free < 150e9:
+        pytest.skip("needs a 180 GB device")
+    k0s = 8.0
+    prm = inputs.iso_params(1.0, k0=k0s)
+    Q = inputs.iso_turbulence(n, 5, 1.0, k0s, device=dev).contiguous()
+    q0 = Q.sum(dim=(1, 2, 3)).cpu().numpy()
+    torch.cuda.empty_cache()
+    free, _ = torch.cuda.mem_get_info(dev)
+    nodes = inputs.cartesian_nodes(n)
+    h = 2.0 * np.pi / n
+    if n == 384:
+        budget = int(free - 42e9)                       # leaves room for the 36 GB of get_state outputs
+    else:
+        budget = (3 * 80 + 5) * n ** 3 * 8 + 14 * (480 + 360) * n * n * 8 + (1 << 20)      # 14 slots -> slab depth 12
+    s = binding.Solver(nodes, binding.make_params(**prm, nonlinear=1), device=dev, budget_bytes=budget)
+    S = int(binding.lib().cgks_slab_depth(s._h))
+    assert 2 <= S < n
+    s.set_state(Q)
+    rng = np.random.default_rng(11)
+    los = [(n - 9, n - 20, n - 3), (S - 14, 5, 17)] + [tuple(int(v) for v in rng.integers(0, n, 3)) for _ in range(nblocks - 2)]
+    blocks = [(lo, _block(Q, lo, 28)) for lo in los]
+    del Q
+    # one dt for both sides: the smallest CFL = 0.4 step of the sampled blocks (oracle formula on each block)
+    bn = inputs.cartesian_nodes(28, 0.0, 28 * h)
+    dts = []
+    for lo, qb in blocks:
+        o = ref.RefSolver(bn, ref.make_params(**prm, nonlinear=1)); o.set_state(qb); dts.append(o.compute_dt(0.4)); o.close()
+    dt = min(dts)
+    s.step(dt); s.status()
+    Qg, Gg, Dg = s.get_state()
+    worst = 0.0
+    for lo, qb in blocks:
+        o = ref.RefSolver(bn, ref.make_params(**prm, nonlinear=1)); o.set_state(qb); o.step(dt)
+        Qo, Go, Do = o.get_state(); o.close()
+        inner = (slice(None),) + (slice(6, 22),) * 3
+        inner2 = (slice(None), slice(None)) + (slice(6, 22),) * 3
+        lo_in = tuple(l + 6 for l in lo)
+        gpu = (_block(Qg, lo_in, 16), _block(Gg, lo_in, 16), _block(Dg, lo_in, 16))
+        orc = (Qo[inner], Go[inner2], Do[inner2])
+        errs = parity.field_errors(gpu, orc, inputs.cartesian_nodes(16, 0.0, 16 * h), qb[inner])
+        w = max(errs, key=errs.get)
+        assert errs[w] <= TOL_1, (lo, w, errs[w])
+        worst = max(worst, errs[w])
+    # whole-mesh property at any size: conservation to round-off
+    tot = Qg.sum(dim=(1, 2, 3)).cpu().numpy()
+    np.testing.assert_allclose(tot, q0, rtol=1e-12, atol=1e-6 * n ** 3 * 1e-6)
+    s.close()
+    print("worst sampled-block error", worst)
