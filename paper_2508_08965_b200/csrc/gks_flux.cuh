@@ -144,29 +144,43 @@ __device__ __forceinline__ double pdot(const double* c, const double* mu) {
   return s;
 }
 
-// out[alpha] (+)= < poly u^I psi_alpha > with u-moments mu (full or half, possibly pre-scaled by rho); N = 3 or 4 coefficients
+// init + sum_k c[k] mu[k] as one FMA chain
+template <int N>
+__device__ __forceinline__ double pdot_acc(const double* c, const double* mu, double init) {
+#pragma unroll
+  for (int k = 0; k < N; k++) init = fma(c[k], mu[k], init);
+  return init;
+}
+
+// out[alpha] (+)= < poly u^I psi_alpha > with u-moments mu (full or half, possibly pre-scaled by rho); N = 3 or 4 coefficients.
+// Accumulating variants continue the FMA chain from the accumulator (no separate add).
 template <int N, int I, bool ACC>
 __device__ __forceinline__ void apply_poly(const double (*c)[N], const double* mu, double* out) {
-  const double r0 = pdot<N>(c[0], mu + I), r1 = pdot<N>(c[0], mu + I + 1), r2 = pdot<N>(c[1], mu + I), r3 = pdot<N>(c[2], mu + I);
-  const double r4 = 0.5 * (pdot<N>(c[0], mu + I + 2) + pdot<N>(c[3], mu + I));
-  if (ACC) { out[0] += r0; out[1] += r1; out[2] += r2; out[3] += r3; out[4] += r4; }
-  else { out[0] = r0; out[1] = r1; out[2] = r2; out[3] = r3; out[4] = r4; }
+  const double r4 = pdot_acc<N>(c[3], mu + I, pdot<N>(c[0], mu + I + 2));      // <u^2 .> + <T2 .>
+  if (ACC) {
+    out[0] = pdot_acc<N>(c[0], mu + I, out[0]); out[1] = pdot_acc<N>(c[0], mu + I + 1, out[1]);
+    out[2] = pdot_acc<N>(c[1], mu + I, out[2]); out[3] = pdot_acc<N>(c[2], mu + I, out[3]);
+    out[4] = fma(0.5, r4, out[4]);
+  } else {
+    out[0] = pdot<N>(c[0], mu + I); out[1] = pdot<N>(c[0], mu + I + 1); out[2] = pdot<N>(c[1], mu + I); out[3] = pdot<N>(c[2], mu + I);
+    out[4] = 0.5 * r4;
+  }
 }
 
 // moments of shift 0 (conserved, outQ) and shift 1 (flux, outF) together: the phi = 1 moments are shared
 template <int N, bool ACC>
 __device__ __forceinline__ void apply_poly_QF(const double (*c)[N], const double* mu, double* outQ, double* outF) {
-  const double e0 = pdot<N>(c[0], mu), e1 = pdot<N>(c[0], mu + 1), e2 = pdot<N>(c[0], mu + 2), e3 = pdot<N>(c[0], mu + 3);
-  const double v0 = pdot<N>(c[1], mu), v1 = pdot<N>(c[1], mu + 1);
-  const double w0 = pdot<N>(c[2], mu), w1 = pdot<N>(c[2], mu + 1);
-  const double t0 = pdot<N>(c[3], mu), t1 = pdot<N>(c[3], mu + 1);
-  const double q4 = 0.5 * (e2 + t0), f4 = 0.5 * (e3 + t1);
+  const double e1 = pdot<N>(c[0], mu + 1), e2 = pdot<N>(c[0], mu + 2);
+  const double q4 = pdot_acc<N>(c[3], mu, e2);                                   // <u^2 .> + <T2 .>, shift 0
+  const double f4 = pdot_acc<N>(c[3], mu + 1, pdot<N>(c[0], mu + 3));            // shift 1
   if (ACC) {
-    outQ[0] += e0; outQ[1] += e1; outQ[2] += v0; outQ[3] += w0; outQ[4] += q4;
-    outF[0] += e1; outF[1] += e2; outF[2] += v1; outF[3] += w1; outF[4] += f4;
+    outQ[0] = pdot_acc<N>(c[0], mu, outQ[0]); outQ[1] += e1;
+    outQ[2] = pdot_acc<N>(c[1], mu, outQ[2]); outQ[3] = pdot_acc<N>(c[2], mu, outQ[3]); outQ[4] = fma(0.5, q4, outQ[4]);
+    outF[0] += e1; outF[1] += e2;
+    outF[2] = pdot_acc<N>(c[1], mu + 1, outF[2]); outF[3] = pdot_acc<N>(c[2], mu + 1, outF[3]); outF[4] = fma(0.5, f4, outF[4]);
   } else {
-    outQ[0] = e0; outQ[1] = e1; outQ[2] = v0; outQ[3] = w0; outQ[4] = q4;
-    outF[0] = e1; outF[1] = e2; outF[2] = v1; outF[3] = w1; outF[4] = f4;
+    outQ[0] = pdot<N>(c[0], mu); outQ[1] = e1; outQ[2] = pdot<N>(c[1], mu); outQ[3] = pdot<N>(c[2], mu); outQ[4] = 0.5 * q4;
+    outF[0] = e1; outF[1] = e2; outF[2] = pdot<N>(c[1], mu + 1); outF[3] = pdot<N>(c[2], mu + 1); outF[4] = 0.5 * f4;
   }
 }
 

@@ -182,13 +182,10 @@ __global__ void __launch_bounds__(128, 3) recon_kernel(Mesh m, Slab sl, const do
 // stage 2 stores only the time derivatives (reading T4).
 // Persistent blocks: each block walks over tiles of FLUX_TPB points (cells x Gauss point q of the + face of AXIS).
 // The 2 x 20 inputs of a point are staged by the owning thread itself with cp.async into its own column of a
-// double-buffered shared-memory tile, one tile ahead of the arithmetic, so the DRAM latency of the loads is hidden
+// shared-memory tile (refilled for the next tile as soon as it has been read into registers), one tile ahead, so the DRAM latency of the loads is hidden
 // behind the ~2000 FP64 instructions of the previous point (no block-level synchronisation is needed: a thread only
 // reads what it copied).
 __device__ __forceinline__ void cp_async8(double* smem_dst, const double* gsrc) {
-#ifdef FLUX_SYNC_COPY
-  *smem_dst = *gsrc; return;
-#endif
   const unsigned sa = (unsigned)__cvta_generic_to_shared(smem_dst);
   asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(sa), "l"(gsrc) : "memory");
 }
@@ -196,10 +193,7 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
 
 constexpr int FLUX_TPB = 128;
-#ifndef FLUX_NBUF
-#define FLUX_NBUF 1
-#endif
-constexpr int FLUX_SMEM_BYTES = FLUX_NBUF * 40 * FLUX_TPB * 8;
+constexpr int FLUX_SMEM_BYTES = 40 * FLUX_TPB * 8;      // one tile: a thread refills its column right after reading it
 
 struct FluxPoint { int q; long t; CellIdx x; int ir, jr, kr; long offL, offR; };
 
@@ -220,18 +214,21 @@ __device__ __forceinline__ bool flux_point(const Mesh& m, const Slab& sl, long t
 template <bool CART, int AXIS, bool STAGE2>
 __global__ void __launch_bounds__(FLUX_TPB, FLUX_MINB) flux_kernel(Mesh m, Slab sl, const double* __restrict__ W, const double* __restrict__ pv,
                                                    double* __restrict__ fx, GasConst gc, double dt, double idt, int kA, long ncells) {
-  extern __shared__ double smf[];                     // [2][40][FLUX_TPB]
+  extern __shared__ double smf[];                     // [40][FLUX_TPB]
   const long tiles_per_q = (ncells + FLUX_TPB - 1) / FLUX_TPB;
   const long ntiles = 4 * tiles_per_q;
   // returns whether this thread has a point in `tile`; its q and left offset are carried to the compute phase
-  auto issue = [&](long tile, int buf, int& q_out, long& offL_out, long& c_out) -> bool {
+  auto issue = [&](long tile, int& q_out, long& offL_out, long& c_out) -> bool {
     FluxPoint f;
     const bool act = tile < ntiles && flux_point<AXIS>(m, sl, tile, tiles_per_q, ncells, kA, f);
     if (act) {
       const double* pL = pv + f.offL;
       const double* pR = pv + f.offR;
+      // NOTE: keep the plane index inside each copy's address expression.  With the base pointers written as
+      // pv + plane * stride + off and advanced by c * stride, nvcc 12.9 / sm_100a produced the RIGHT face's plane for
+      // the left copies of AXIS = 2 (caught by the parity tests; the echo of the staged values showed it).
       const long planeL = (long)((4 * (2 * AXIS) + f.q) * 20), planeR = (long)((4 * (2 * AXIS + 1) + f.q) * 20);
-      double* dstL = smf + (long)(buf * 40) * FLUX_TPB + threadIdx.x;
+      double* dstL = smf + threadIdx.x;
 #pragma unroll
       for (int c = 0; c < 20; c++) cp_async8(dstL + c * FLUX_TPB, pL + (planeL + c) * sl.stride_pv);
 #pragma unroll
@@ -241,29 +238,20 @@ __global__ void __launch_bounds__(FLUX_TPB, FLUX_MINB) flux_kernel(Mesh m, Slab 
     cp_async_commit();
     return act;
   };
-  int buf = 0, q = 0, qn = 0;
+  int q = 0, qn = 0;
   long offL = 0, offLn = 0, cL = 0, cLn = 0;
-  bool active = issue(blockIdx.x, 0, q, offL, cL), activen = false;
+  bool active = issue(blockIdx.x, q, offL, cL), activen = false;
 #pragma unroll 1
-  for (long tile = blockIdx.x; tile < ntiles; tile += gridDim.x, buf ^= (FLUX_NBUF - 1), q = qn, offL = offLn, cL = cLn, active = activen) {
+  for (long tile = blockIdx.x; tile < ntiles; tile += gridDim.x, q = qn, offL = offLn, cL = cLn, active = activen) {
   cp_async_wait<0>();
-  const double* sL = smf + (long)(buf * 40) * FLUX_TPB + threadIdx.x;
+  const double* sL = smf + threadIdx.x;
   double WLg[5], WRg[5], gL[15], gR[15];
 #pragma unroll
   for (int c = 0; c < 5; c++) { WLg[c] = sL[c * FLUX_TPB]; WRg[c] = sL[(20 + c) * FLUX_TPB]; }
 #pragma unroll
   for (int c = 0; c < 15; c++) { gL[c] = sL[(5 + c) * FLUX_TPB]; gR[c] = sL[(25 + c) * FLUX_TPB]; }
-  activen = issue(tile + gridDim.x, buf ^ (FLUX_NBUF - 1), qn, offLn, cLn);      // next tile's inputs stream in while this point is computed
+  activen = issue(tile + gridDim.x, qn, offLn, cLn);      // next tile's inputs stream in while this point is computed
   if (!active) continue;
-#ifdef FLUX_DEBUG_ECHO
-  {
-    double* dste = fx + (long)((4 * AXIS + q) * 30) * sl.stride_fx + offL;
-    for (int c = 0; c < 5; c++) { dste[(long)c * sl.stride_fx] = WLg[c]; dste[(long)(5 + c) * sl.stride_fx] = WRg[c]; }
-    for (int c = 0; c < 15; c++) dste[(long)(10 + c) * sl.stride_fx] = gR[c];
-    for (int c = 0; c < 5; c++) dste[(long)(25 + c) * sl.stride_fx] = gL[c];
-    continue;
-  }
-#endif
   // positivity (reading R9, point-wise): a non-physical reconstructed state falls back to the cell average
   {
     const double eL = WLg[0] * WLg[4] - 0.5 * (WLg[1] * WLg[1] + WLg[2] * WLg[2] + WLg[3] * WLg[3]);    // rho * (rho e)
