@@ -789,6 +789,87 @@ int cgks_ref_step(cgks_ref_ctx* c, double dt) {
   return check_physical(c, c->Q, "stage 2");
 }
 
+/* ------------------------------------------------------------------ */
+/* Diagnostics: volume-averaged kinetic energy and   */
+/* enstrophy, "calculated by numerical quadrature, and the velocity     */
+/* derivative values at quadrature points are obtained by the compact   */
+/* reconstruction".  Reading X1: 2x2x2 Gauss      */
+/* points (+-g,+-g,+-g) of the reference cell, weights |Omega|/8, the   */
+/* scheme's own (blended, Eq. 16) polynomial of the conservative        */
+/* variables, U = m/rho, the solver's viscosity law for mu, point-wise  */
+/* positivity fallback R9.  Returns the integrals divided by |Omega|    */
+/* (rho_0 = 1 is left to the caller).                                   */
+/* ------------------------------------------------------------------ */
+int cgks_ref_diagnostics(cgks_ref_ctx* c, double* Ek_out, double* ens_out) {
+  const long n = c->n; const double g = 0.5 / sqrt(3.0);
+  double Ek = 0, ens = 0, vtot = 0;
+  for (int k = 0; k < c->nk; k++) for (int j = 0; j < c->nj; j++) for (int i = 0; i < c->ni; i++) {
+    long ci = cidx(c, i, j, k);
+    const double* J = c->J0 + 9 * ci; const double* Ji = c->J0inv + 9 * ci;
+    double val[8][5], grd[8][5][3];
+    for (int v = 0; v < NV; v++) {
+      const double* q = c->Q + v * n;
+      double q0 = q[ci], d[ND];
+      for (int m = 0; m < 6; m++) d[m] = q[cidx(c, i + g_face_off[m][0], j + g_face_off[m][1], k + g_face_off[m][2])] - q0;
+      for (int e = 0; e < 12; e++) d[6 + e] = q[cidx(c, i + g_edge_off[e][0], j + g_edge_off[e][1], k + g_edge_off[e][2])] - q0;
+      for (int m = 0; m < 6; m++) {
+        long nb = cidx(c, i + g_face_off[m][0], j + g_face_off[m][1], k + g_face_off[m][2]);
+        for (int a = 0; a < 3; a++) {
+          double s = 0; for (int r = 0; r < 3; r++) s += J[3 * r + a] * c->G[(v * 3 + r) * n + nb];
+          d[18 + 3 * m + a] = 2.0 * s;
+        }
+      }
+      for (int e = 0; e < 12; e++) {
+        long nb = cidx(c, i + g_edge_off[e][0], j + g_edge_off[e][1], k + g_edge_off[e][2]);
+        double gr[3];
+        for (int a = 0; a < 3; a++) { double s = 0; for (int r = 0; r < 3; r++) s += J[3 * r + a] * c->G[(v * 3 + r) * n + nb]; gr[a] = s; }
+        d[36 + 2 * e] = gr[g_edge_axis[e]];
+        d[36 + 2 * e + 1] = (g_edge_off[e][0] * gr[0] + g_edge_off[e][1] * gr[1] + g_edge_off[e][2] * gr[2]) / sqrt(2.0);
+      }
+      for (int s = 0; s < 12; s++) d[60 + s] = 3.0 * c->D[(v * 12 + s) * n + ci];
+      double a[NB], b[18], chi, om[6], fval[NGP], fgref[NGP * 3];
+      cgks_ref_recon_reference(&c->prm, d, a, b, &chi, om, fval, fgref);
+      for (int p = 0; p < 8; p++) {
+        double x[3] = { (p & 4) ? g : -g, (p & 2) ? g : -g, (p & 1) ? g : -g };
+        double v4 = 0, g4[3] = { 0, 0, 0 }, v1 = 0, g1[3] = { 0, 0, 0 };
+        for (int bb = 0; bb < NB; bb++) {
+          v4 += a[bb] * basis_pt(g_didx[bb], x);
+          for (int ax = 0; ax < 3; ax++) g4[ax] += a[bb] * basis_dpt(g_didx[bb], x, ax);
+        }
+        for (int m = 0; m < 6; m++) {
+          v1 += om[m] * (b[3 * m] * x[0] + b[3 * m + 1] * x[1] + b[3 * m + 2] * x[2]);
+          for (int ax = 0; ax < 3; ax++) g1[ax] += om[m] * b[3 * m + ax];
+        }
+        val[p][v] = q0 + chi * v4 + (1.0 - chi) * v1;
+        double gr[3];
+        for (int ax = 0; ax < 3; ax++) gr[ax] = chi * g4[ax] + (1.0 - chi) * g1[ax];
+        for (int r = 0; r < 3; r++) grd[p][v][r] = Ji[0 * 3 + r] * gr[0] + Ji[1 * 3 + r] * gr[1] + Ji[2 * 3 + r] * gr[2];
+      }
+    }
+    for (int p = 0; p < 8; p++) {
+      double rho = val[p][0], pe = val[p][4] - 0.5 * (val[p][1] * val[p][1] + val[p][2] * val[p][2] + val[p][3] * val[p][3]) / rho;
+      if (!(rho > 0.0) || !(pe > 0.0)) {
+        for (int v = 0; v < NV; v++) { val[p][v] = c->Q[v * n + ci]; for (int r = 0; r < 3; r++) grd[p][v][r] = 0.0; }
+        rho = val[p][0];
+        pe = val[p][4] - 0.5 * (val[p][1] * val[p][1] + val[p][2] * val[p][2] + val[p][3] * val[p][3]) / rho;
+      }
+      double U[3] = { val[p][1] / rho, val[p][2] / rho, val[p][3] / rho };
+      double dU[3][3];   /* dU[a][r] = d U_a / d x_r = (d m_a - U_a d rho)/rho */
+      for (int a = 0; a < 3; a++) for (int r = 0; r < 3; r++) dU[a][r] = (grd[p][1 + a][r] - U[a] * grd[p][0][r]) / rho;
+      double w[3] = { dU[2][1] - dU[1][2], dU[0][2] - dU[2][0], dU[1][0] - dU[0][1] };
+      double pres = (c->prm.gamma - 1.0) * pe;
+      double mu = c->prm.mu_ref;
+      if (c->prm.mu_ref > 0.0 && c->prm.visc_omega != 0.0) mu *= pow((pres / rho) / c->prm.T_ref, c->prm.visc_omega);
+      double wq = c->vol[ci] / 8.0;
+      Ek += wq * 0.5 * rho * (U[0] * U[0] + U[1] * U[1] + U[2] * U[2]);
+      ens += wq * mu * (w[0] * w[0] + w[1] * w[1] + w[2] * w[2]);
+    }
+    vtot += c->vol[ci];
+  }
+  *Ek_out = Ek / vtot; *ens_out = ens / vtot;
+  return 0;
+}
+
 /* time step (reading S3): dt = CFL / max_cells sum_d (|U.n_d| + c)/h_d, h_d = |Omega|/S_d;
    viscous cap dt <= CFL min_d h_d^2 / (3 nu).  The sum over the three index directions is the
    reading that reproduces Table 1 (S3). */

@@ -44,6 +44,7 @@ void   cgks_ref_destroy(cgks_ref_ctx*);
 int    cgks_ref_set_state(cgks_ref_ctx*, const double* Q, const double* G, const double* D);
 int    cgks_ref_get_state(cgks_ref_ctx*, double* Q, double* G, double* D);
 int    cgks_ref_compute_dt(cgks_ref_ctx*, double cfl, double* dt);
+int    cgks_ref_diagnostics(cgks_ref_ctx*, double* Ek, double* enstrophy);   /* PAPER.md:428-454, reading X1 */
 int    cgks_ref_step(cgks_ref_ctx*, double dt);      /* 0 ok, -4 non-physical cell average */
 const char* cgks_ref_last_error(const cgks_ref_ctx*);
 

@@ -50,6 +50,7 @@ def lib():
         L.cgks_ref_recon_reference.argtypes = [C.POINTER(Params)] + [_dp] * 7
         L.cgks_ref_smoothness.argtypes = [_dp, _dp]
         L.cgks_ref_reconstruct.argtypes = [C.c_void_p, _dp, _dp]
+        L.cgks_ref_diagnostics.argtypes = [C.c_void_p, _dp, _dp]
         L.cgks_ref_debug_flux.argtypes = [C.c_void_p, C.c_double, _dp]
         L.cgks_ref_flux_point.argtypes = [C.POINTER(Params), C.c_double] + [_dp] * 7
         L.cgks_ref_moments.argtypes = [C.c_double, C.c_double, _dp, _dp, _dp]
@@ -167,6 +168,12 @@ class RefSolver:
         rc = lib().cgks_ref_step(self._h, float(dt))
         if rc:
             raise FloatingPointError(lib().cgks_ref_last_error(self._h).decode())
+
+    def diagnostics(self):
+        """(E_k, enstrophy) of PAPER.md:428-454, divided by |Omega| (rho_0 = 1)."""
+        ek = np.zeros(1); en = np.zeros(1)
+        lib().cgks_ref_diagnostics(self._h, _p(ek), _p(en))
+        return float(ek[0]), float(en[0])
 
     def reconstruct(self):
         pv = np.zeros((self.nk, self.nj, self.ni, NGP, 20)); chi = np.zeros((5, self.nk, self.nj, self.ni))

@@ -290,13 +290,15 @@ def emit_group(name, nloc, orbits):
     return "\n".join(L)
 
 
-def emit_eval_axis(ax, B):
+def emit_eval_axis(ax, B, volume=False):
     """Value and reference gradient at the 8 Gauss points of the face pair of axis ax: out[4*(4*sgn + 2*a + b) + kappa],
-    sgn = 0 for the + face; (a, b) select -g/+g on the two other axes (ascending); kappa = 0 value, 1..3 d/dxi_r."""
+    sgn = 0 for the + face; (a, b) select -g/+g on the two other axes (ascending); kappa = 0 value, 1..3 d/dxi_r.
+    volume=True: the 8 interior Gauss points (+-g, +-g, +-g) of the 2x2x2 rule instead (ax = 0; sgn = 0 selects +g)."""
     o1, o2 = other_axes(ax)
-    xs = [0.0, 0.0, 0.0]; xs[ax] = 0.5; xs[o1] = G; xs[o2] = G
+    xs = [0.0, 0.0, 0.0]; xs[ax] = G if volume else 0.5; xs[o1] = G; xs[o2] = G
     one = np.array(1.0)
-    L = ["__device__ __forceinline__ void recon_eval_axis%d(const double* __restrict__ a, double* __restrict__ out) {" % ax]
+    L = ["__device__ __forceinline__ void recon_eval_%s(const double* __restrict__ a, double* __restrict__ out) {"
+         % ("volume" if volume else "axis%d" % ax)]
     for kap in range(4):
         sums = {}
         for b, d in enumerate(B):
@@ -385,6 +387,7 @@ def generate(path):
             emit_quadform("recon_IS34", Gram[2] + Gram[3])]
     for ax in range(3):
         out.append(emit_eval_axis(ax, B))
+    out.append(emit_eval_axis(0, B, volume=True))
     out.append("")
     with open(path, "w") as f:
         f.write("\n".join(out))
