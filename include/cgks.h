@@ -78,6 +78,12 @@ int cgks_compute_dt(cgks_ctx*, double cfl, double* dt_host);
 /* One two-stage fourth-order step of size dt.  Asynchronous. */
 int cgks_step(cgks_ctx*, double dt);
 
+/* Diagnostics of the current state: volume-averaged kinetic energy E_k = int rho |U|^2/2 dV / |Omega| and
+   enstrophy int mu |curl U|^2 dV / |Omega| (rho_0 = 1), by the 2x2x2 Gauss rule on every cell with values and velocity
+   derivatives from the compact reconstruction (the scheme's own polynomial, Eq. 16; reading X1); mu is the
+   solver's viscosity law.  Synchronises; overwrites the chi tap and the slab buffers.  Host pointers. */
+int cgks_diagnostics(cgks_ctx*, double* ek_host, double* enstrophy_host);
+
 /* Synchronises and returns CGKS_OK, CGKS_ECUDA or CGKS_ENONPHYSICAL for the work enqueued so far. */
 int cgks_status(cgks_ctx*);
 

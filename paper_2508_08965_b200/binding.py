@@ -47,6 +47,7 @@ def lib():
         L.cgks_compute_dt.argtypes = [_vp, C.c_double, C.POINTER(C.c_double)]
         L.cgks_step.argtypes = [_vp, C.c_double]
         L.cgks_status.argtypes = [_vp]
+        L.cgks_diagnostics.argtypes = [_vp, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.cgks_run_host.argtypes = [_vp, _vp, _vp, _vp, C.c_double, C.c_int, _vp, _vp, _vp]
         L.cgks_launch_count.argtypes = [_vp]; L.cgks_launch_count.restype = C.c_long
         L.cgks_slab_depth.argtypes = [_vp]
@@ -172,6 +173,12 @@ class Solver:
 
     def step(self, dt):
         self._check(lib().cgks_step(self._h, float(dt)))
+
+    def diagnostics(self):
+        """(E_k, enstrophy) of the current state, divided by |Omega|."""
+        ek = C.c_double(0.0); en = C.c_double(0.0)
+        self._check(lib().cgks_diagnostics(self._h, C.byref(ek), C.byref(en)))
+        return ek.value, en.value
 
     def status(self):
         self._check(lib().cgks_status(self._h))

@@ -362,6 +362,41 @@ extern "C" int cgks_debug_stage(cgks_ctx* c, double dt, double* d_pv, double* d_
   return CGKS_OK;
 }
 
+// ---- diagnostics ---------------------------------------------------------------------------------
+template <bool CART>
+static void run_diagnostics(cgks_ctx* c, double* d_acc) {
+  const Mesh& m = c->mesh;
+  const double* Win = c->W[c->cur];
+  ReconPrm rp{ c->prm.nonlinear, c->prm.geno_C, c->prm.geno_eps, 1.0 / tanh(c->prm.geno_C), c->prm.gamma };
+  DiagPrm dp{ c->prm.gamma, c->prm.mu_ref, c->prm.visc_omega, 1.0 / c->prm.T_ref };
+  Slab sl; sl.slots_pv = c->slots_pv; sl.slots_fx = c->slots_fx;
+  sl.stride_pv = (long)c->slots_pv * m.plane; sl.stride_fx = (long)c->slots_fx * m.plane;
+  const int S = c->S >= m.nk ? m.nk : c->S;
+  for (int k0 = 0; k0 < m.nk; k0 += S) {
+    const int cnt = (k0 + S < m.nk) ? S : m.nk - k0;
+    sl.kbase = k0;
+    const long nt = (long)cnt * m.plane;
+    const unsigned nb = (unsigned)((nt + TPB - 1) / TPB);
+    { Timed t(c, KC_OTHER); recon_kernel<CART, true><<<dim3(nb, 5), TPB, 0, c->stream>>>(m, sl, Win, c->pv, nullptr, rp, k0, nt, c->d_flags + 3); }
+    { Timed t(c, KC_OTHER); diag_kernel<CART><<<nb, TPB, 0, c->stream>>>(m, sl, Win, c->pv, dp, k0, nt, c->fx); }     // fx = scratch for the partials
+    { Timed t(c, KC_OTHER); diag_reduce_kernel<<<1, 256, 0, c->stream>>>(c->fx, (long)nb, d_acc); }
+  }
+}
+
+extern "C" int cgks_diagnostics(cgks_ctx* c, double* ek_host, double* enstrophy_host) {
+  if (!c || !ek_host || !enstrophy_host) return CGKS_EINVAL;
+  double* d_acc = c->chi;                 // 3 doubles of the chi buffer serve as the accumulator (chi is a diagnostic tap only)
+  CK(cudaMemsetAsync(d_acc, 0, 3 * sizeof(double), c->stream));
+  if (c->mesh.cart) run_diagnostics<true>(c, d_acc); else run_diagnostics<false>(c, d_acc);
+  double acc[3] = { 0, 0, 0 };
+  CK(cudaMemcpyAsync(acc, d_acc, sizeof acc, cudaMemcpyDeviceToHost, c->stream));
+  CK(cudaStreamSynchronize(c->stream));
+  CK(cudaGetLastError());
+  if (!(acc[2] > 0.0)) return fail(c, CGKS_ECUDA, "diagnostics: zero volume");
+  *ek_host = acc[0] / acc[2]; *enstrophy_host = acc[1] / acc[2];
+  return CGKS_OK;
+}
+
 extern "C" int cgks_set_profiling(cgks_ctx* c, int on) {
   if (!c) return CGKS_EINVAL;
   c->profiling = on ? 1 : 0;

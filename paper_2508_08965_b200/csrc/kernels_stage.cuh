@@ -80,7 +80,9 @@ __device__ __forceinline__ void recon_gather_axis(const ReconCell<CART>& rc, con
   }
 }
 
-template <bool CART>
+// VOLUME = true: the same polynomial evaluated at the 8 interior points (+-g, +-g, +-g) of the 2x2x2 Gauss rule instead
+// (pv planes 0..7, used by the diagnostics of PAPER.md:428-454).
+template <bool CART, bool VOLUME = false>
 __global__ void __launch_bounds__(128, 3) recon_kernel(Mesh m, Slab sl, const double* __restrict__ W, double* __restrict__ pv,
                                                     double* __restrict__ chi_out, ReconPrm rp, int kA, long nthreads,
                                                     int* __restrict__ flag) {
@@ -172,9 +174,88 @@ __global__ void __launch_bounds__(128, 3) recon_kernel(Mesh m, Slab sl, const do
       for (int r = 0; r < 3; r++) dst[(long)(5 + 3 * v + r) * sl.stride_pv] = g[r];
     }
   };
+  if (VOLUME) { double o[32]; recon_eval_volume(a, o); store_axis(0, o); return; }
   { double o[32]; eval_axis<0>(a, o); store_axis(0, o); }
   { double o[32]; eval_axis<1>(a, o); store_axis(1, o); }
   { double o[32]; eval_axis<2>(a, o); store_axis(2, o); }
+}
+
+// ------------------------------------------------------------------------------------------------ diagnostics
+// E_k = int rho |U|^2/2 dV / |Omega|, enstrophy = int mu |curl U|^2 dV / |Omega| by the 2x2x2 Gauss rule
+// with the reconstructed polynomial (reading X1).  Thread per cell over the 8 points staged in pv by
+// recon_kernel<CART, true>; deterministic block tree reduction, one partial triple (E_k, enstrophy, volume) per block.
+struct DiagPrm { double gamma, mu_ref, omega, inv_T_ref; };
+
+template <bool CART>
+__global__ void __launch_bounds__(128) diag_kernel(Mesh m, Slab sl, const double* __restrict__ W, const double* __restrict__ pv,
+                                                   DiagPrm dp, int kA, long nthreads, double* __restrict__ partial) {
+  __shared__ double red[3][128];
+  const long t = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  double ek = 0.0, en = 0.0, vol = 0.0;
+  if (t < nthreads) {
+    const CellIdx x = cell_of(m, t, kA);
+    const long off = (long)slot_of(m, sl, x.k) * m.plane + x.ij;
+    vol = CART ? m.h[0] * m.h[1] * m.h[2] : m.met[MET_VOL * m.n + x.c];
+#pragma unroll 1
+    for (int p = 0; p < 8; p++) {
+      const double* src = pv + (long)(p * 20) * sl.stride_pv + off;
+      double w[5], g[4][3];
+#pragma unroll
+      for (int c = 0; c < 5; c++) w[c] = src[(long)c * sl.stride_pv];
+#pragma unroll
+      for (int c = 0; c < 4; c++)
+#pragma unroll
+        for (int r = 0; r < 3; r++) g[c][r] = src[(long)(5 + 3 * c + r) * sl.stride_pv];
+      double pe = w[4] - 0.5 * (w[1] * w[1] + w[2] * w[2] + w[3] * w[3]) / w[0];
+      if (!(w[0] > 0.0) || !(pe > 0.0)) {      // positivity fallback (reading R9): cell average, zero gradient
+#pragma unroll
+        for (int c = 0; c < 5; c++) w[c] = W[(long)c * m.n + x.c];
+#pragma unroll
+        for (int c = 0; c < 4; c++) { g[c][0] = 0.0; g[c][1] = 0.0; g[c][2] = 0.0; }
+        pe = w[4] - 0.5 * (w[1] * w[1] + w[2] * w[2] + w[3] * w[3]) / w[0];
+      }
+      const double ir = 1.0 / w[0];
+      const double U[3] = { w[1] * ir, w[2] * ir, w[3] * ir };
+      double dU[3][3];      // dU[a][r] = d U_a / d x_r
+#pragma unroll
+      for (int a = 0; a < 3; a++)
+#pragma unroll
+        for (int r = 0; r < 3; r++) dU[a][r] = (g[1 + a][r] - U[a] * g[0][r]) * ir;
+      const double c0 = dU[2][1] - dU[1][2], c1 = dU[0][2] - dU[2][0], c2 = dU[1][0] - dU[0][1];
+      double mu = dp.mu_ref;
+      if (dp.mu_ref > 0.0 && dp.omega != 0.0) mu *= pow(((dp.gamma - 1.0) * pe * ir) * dp.inv_T_ref, dp.omega);
+      ek += 0.5 * w[0] * (U[0] * U[0] + U[1] * U[1] + U[2] * U[2]);
+      en += mu * (c0 * c0 + c1 * c1 + c2 * c2);
+    }
+    ek *= 0.125 * vol; en *= 0.125 * vol;
+  }
+  red[0][threadIdx.x] = ek; red[1][threadIdx.x] = en; red[2][threadIdx.x] = vol;
+  __syncthreads();
+  for (int s2 = 64; s2 > 0; s2 >>= 1) {
+    if (threadIdx.x < s2) {
+#pragma unroll
+      for (int c = 0; c < 3; c++) red[c][threadIdx.x] += red[c][threadIdx.x + s2];
+    }
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) { partial[3 * (long)blockIdx.x] = red[0][0]; partial[3 * (long)blockIdx.x + 1] = red[1][0]; partial[3 * (long)blockIdx.x + 2] = red[2][0]; }
+}
+
+// sums the per-block partial triples in a fixed order (one block) and ADDS them to acc[0..2]
+__global__ void __launch_bounds__(256) diag_reduce_kernel(const double* __restrict__ partial, long nblocks, double* __restrict__ acc) {
+  __shared__ double red[3][256];
+  double s0 = 0.0, s1 = 0.0, s2 = 0.0;
+  for (long b = threadIdx.x; b < nblocks; b += 256) { s0 += partial[3 * b]; s1 += partial[3 * b + 1]; s2 += partial[3 * b + 2]; }
+  red[0][threadIdx.x] = s0; red[1][threadIdx.x] = s1; red[2][threadIdx.x] = s2;
+  __syncthreads();
+  for (int w = 128; w > 0; w >>= 1) {
+    if (threadIdx.x < w) {
+#pragma unroll
+      for (int c = 0; c < 3; c++) red[c][threadIdx.x] += red[c][threadIdx.x + w];
+    }
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) { acc[0] += red[0][0]; acc[1] += red[1][0]; acc[2] += red[2][0]; }
 }
 
 // ------------------------------------------------------------------------------------------------ flux

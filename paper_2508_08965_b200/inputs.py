@@ -194,6 +194,13 @@ def workload(name, n=None, k0=None):
         n = n or 64
         nodes = curvilinear_nodes(n)
         return dict(nodes=nodes, Q=taylor_green(nodes), G=None, D=None, params=tgv_params(), nonlinear=1, cfl=0.5, steps=200)
+    if name == "tgv_sup":
+        # the paper's second Taylor-Green workload, Ma = 1.25, Pr = 0.7, nonlinear reconstruction only
+        # (128^3 and 320^3 in the paper); shocklets form from t ~ 3
+        n = n or 128
+        nodes = cartesian_nodes(n)
+        return dict(nodes=nodes, Q=taylor_green(nodes, Ma=1.25), G=None, D=None, params=tgv_params(Ma=1.25, Pr=0.7),
+                    nonlinear=1, cfl=0.5, steps=200)
     if name == "freestream_curv":
         n = n or 64
         nodes = curvilinear_nodes(n)
