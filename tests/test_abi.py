@@ -74,3 +74,18 @@ def test_product_path_does_not_import_the_oracle():
     for fn in os.listdir(os.path.join(ROOT, "paper_2508_08965_b200", "csrc")):
         txt = open(os.path.join(ROOT, "paper_2508_08965_b200", "csrc", fn), errors="ignore").read()
         assert "cgks_ref" not in txt and "oracle/" not in txt.replace("oracle/)", ""), fn
+
+
+def test_generated_headers_are_current(tmp_path):
+    """csrc/recon_gen.cuh and csrc/math_gen.cuh (committed) are exactly what their generators produce, and the
+    symmetry-reduced reconstruction operators reproduce a = M d (numpy emulation of the emitted structure)."""
+    import importlib.util
+    csrc = os.path.join(ROOT, "paper_2508_08965_b200", "csrc")
+    for gen, hdr in (("gen_recon.py", "recon_gen.cuh"), ("gen_math.py", "math_gen.cuh")):
+        spec = importlib.util.spec_from_file_location(gen[:-3], os.path.join(csrc, gen))
+        mod = importlib.util.module_from_spec(spec); spec.loader.exec_module(mod)
+        out = tmp_path / hdr
+        mod.generate(str(out))
+        assert out.read_text() == open(os.path.join(csrc, hdr)).read(), hdr
+        if gen == "gen_recon.py":
+            assert mod.self_check() == 312
