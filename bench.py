@@ -42,7 +42,7 @@ def parse():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=4)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--n", type=int, default=384, help="cells per direction (default: the 384^3 headline config)")
+    ap.add_argument("--n", "--size", dest="n", type=int, default=384, help="cells per direction (default: the 384^3 headline config)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
