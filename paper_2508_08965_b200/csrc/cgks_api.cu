@@ -413,15 +413,20 @@ extern "C" int cgks_kernel_ms(const cgks_ctx* c, int which, double* ms, long* la
 
 // ---- FP64 FMA peak micro-benchmark (roofline denominator check) ------------------------------------------------------
 __global__ void __launch_bounds__(256) dfma_peak_kernel(double* out, int iters, double a, double b) {
-  double x0 = threadIdx.x * 1e-3, x1 = x0 + 1, x2 = x0 + 2, x3 = x0 + 3, x4 = x0 + 4, x5 = x0 + 5, x6 = x0 + 6, x7 = x0 + 7;
-  for (int i = 0; i < iters; i++) {
+  // 8 independent chains per thread, all three operands of every DFMA in distinct, rotating registers
+  double x[8], y[8], z[8];
+#pragma unroll
+  for (int i = 0; i < 8; i++) { x[i] = threadIdx.x * 1e-3 + i; y[i] = a + 1e-9 * i; z[i] = b * (i + 1); }
+  for (int it = 0; it < iters; it++) {
 #pragma unroll
     for (int u = 0; u < 8; u++) {
-      x0 = fma(x0, a, b); x1 = fma(x1, a, b); x2 = fma(x2, a, b); x3 = fma(x3, a, b);
-      x4 = fma(x4, a, b); x5 = fma(x5, a, b); x6 = fma(x6, a, b); x7 = fma(x7, a, b);
+#pragma unroll
+      for (int i = 0; i < 8; i++) x[i] = fma(x[i], y[(i + u) & 7], z[(i + 3 * u) & 7]);
     }
   }
-  const double s = x0 + x1 + x2 + x3 + x4 + x5 + x6 + x7;
+  double s = 0;
+#pragma unroll
+  for (int i = 0; i < 8; i++) s += x[i];
   if (s == 12345.678) out[0] = s;      // never true; keeps the chains alive
 }
 
