@@ -114,8 +114,8 @@ int cgks_get_chi(cgks_ctx*, double* d_chi);
    Needs the whole mesh resident (CGKS_ENOMEM otherwise).  The state is not modified. */
 int cgks_debug_stage(cgks_ctx*, double dt, double* d_pv, double* d_fx);
 
-/* Measures the device's FP64 FMA throughput with a register-resident DFMA micro-benchmark (8 independent chains, distinct operands
-   per thread, 148*8 blocks of 256 threads) on `cuda_stream`; TFLOP/s (FMA = 2 flops) to *tflops (host).
+/* Measures the device's FP64 FMA throughput with a register-resident DFMA micro-benchmark (8 independent chains
+   per thread, three distinct rotating register operands, 148*8 blocks of 256 threads) on `cuda_stream`; TFLOP/s (FMA = 2 flops) to *tflops (host).
    The only call that allocates device memory itself (8 bytes, freed before returning). */
 int cgks_fp64_peak(void* cuda_stream, double* tflops);
 
