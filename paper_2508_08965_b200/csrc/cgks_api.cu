@@ -311,7 +311,8 @@ static void run_stage(cgks_ctx* c, int stage, double dt) {
     const long nt = (long)cnt * m.plane;
     dim3 grid((unsigned)((nt + TPB - 1) / TPB), 5);
     Timed t(c, KC_UPDATE);
-    update_kernel<CART><<<grid, TPB, 0, c->stream>>>(m, sl, c->fx, c->W[c->cur], c->W[c->star], c->W[c->save], dt, kA, nt, stage);
+    if (stage == 1) update_kernel<CART, 1><<<grid, TPB, 0, c->stream>>>(m, sl, c->fx, c->W[c->cur], c->W[c->star], c->W[c->save], dt, kA, nt);
+    else update_kernel<CART, 2><<<grid, TPB, 0, c->stream>>>(m, sl, c->fx, c->W[c->cur], c->W[c->star], c->W[c->save], dt, kA, nt);
   };
   if (c->S >= m.nk) {                       // whole mesh resident: no recomputation
     sl.kbase = 0;

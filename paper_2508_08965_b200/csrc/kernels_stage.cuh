@@ -425,10 +425,11 @@ __global__ void __launch_bounds__(FLUX_TPB, FLUX_MINB) flux_kernel(Mesh m, Slab 
 // Thread per (cell, variable).  Eq. 8-10 and the S2O4 combine.
 //   stage 1: Wstar = stage value at t_n + dt/2;  Wsave = { Q^n + dt L^n + dt^2/6 L_t^n,  G,D sums of V^n }
 //   stage 2: Wsave <- { Wsave.Q + dt^2/3 L_t^*,  Wsave.GD + dt * (G,D sums of Dt^*) }   (in place) = state at t_n+1
-template <bool CART>
+template <bool CART, int STAGE>
 __global__ void __launch_bounds__(128) update_kernel(Mesh m, Slab sl, const double* __restrict__ fx, const double* __restrict__ Wcur,
                                                      double* __restrict__ Wstar, double* __restrict__ Wsave, double dt,
-                                                     int kA, long nthreads, int stage) {
+                                                     int kA, long nthreads) {
+  constexpr int stage = STAGE;
   const long t = (long)blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= nthreads) return;
   const int v = blockIdx.y;
