@@ -215,14 +215,15 @@ def _block(t, lo, size):
     return t.index_select(-3, idx[0]).index_select(-2, idx[1]).index_select(-1, idx[2]).cpu().numpy()
 
 
-@pytest.mark.parametrize("n,nblocks", [(384, 6), (96, 4)])
-def test_full_size_sampled_blocks(n, nblocks):
+@pytest.mark.parametrize("n,nblocks,Ma_t,seed", [(384, 6, 1.0, 5), (96, 4, 1.0, 5), (128, 4, 0.5, 4)])
+def test_full_size_sampled_blocks(n, nblocks, Ma_t, seed):
     """BASELINE.json config 5 at its full size (384^3, the configuration bench.py times: slab pipeline, Cartesian
     kernels), one S2O4 step, checked on sampled 16^3 blocks the oracle can compute on their own: a cell's new state
     depends on cell averages within index distance 6 (bootstrap 2 + two stages of 2), so the oracle run on the periodic
     28^3 block around a sample reproduces the inner 16^3 exactly, whatever happens at the block's own (wrong) periodic
     seam.  Blocks are seeded, and include the periodic seam of the full mesh and a slab boundary of the pipeline.
-    The 96^3 case runs the same check with a workspace that forces a slab depth of 12."""
+    The 96^3 case runs the same check with a workspace that forces a slab depth of 12; the 128^3 case is BASELINE.json
+    config 4 (Ma_t = 0.5, seed 4) at its full size, also through the slab pipeline."""
     import torch
     from oracle import ref
     from paper_2508_08965_b200 import binding
@@ -232,8 +233,8 @@ def test_full_size_sampled_blocks(n, nblocks):
     if n == 384 and free < 150e9:
         pytest.skip("needs a 180 GB device")
     k0s = 8.0
-    prm = inputs.iso_params(1.0, k0=k0s)
-    Q = inputs.iso_turbulence(n, 5, 1.0, k0s, device=dev).contiguous()
+    prm = inputs.iso_params(Ma_t, k0=k0s)
+    Q = inputs.iso_turbulence(n, seed, Ma_t, k0s, device=dev).contiguous()
     q0 = Q.sum(dim=(1, 2, 3)).cpu().numpy()
     torch.cuda.empty_cache()
     free, _ = torch.cuda.mem_get_info(dev)
@@ -337,3 +338,11 @@ def test_long_runs_stay_physical_and_conservative(name, n, steps):
     if name != "iso_sub":
         assert (chi < 0.99).double().mean().item() > 1e-5
     s.close()
+
+
+@pytest.mark.parametrize("name,n,steps", [("tgv", 64, 3), ("tgv_curv", 64, 2), ("freestream_curv", 64, 2)])
+def test_configs_2_and_3_at_full_size(name, n, steps):
+    """BASELINE.json configs 2 and 3 at their full 64^3 size (Cartesian and non-orthogonal mesh), a few S2O4 steps,
+    every field against the oracle element by element."""
+    w = parity.build_case(name, n, 1)
+    _check(w, steps, TOL_1 * steps)
