@@ -56,7 +56,9 @@ typedef struct {
 
 /* Bytes of device workspace for a mesh of ni x nj x nk cells (state, stage buffers, metrics, and the slab buffers
    of reconstructed face values and face fluxes).  `budget_bytes` = 0 asks for the default (largest useful slab up
-   to ~48 GB of slab buffers); otherwise the slab depth is reduced so that the total stays below the budget. */
+   to ~48 GB of slab buffers); otherwise the slab depth is reduced so that the total stays below the budget, and
+   CGKS_ENOMEM is returned when not even a slab of two k-planes fits under it.  (`budget_bytes` is an addition to
+   the call list of SURVEY.md 8(b): the 384^3 case needs the caller to say how much of the device it may take.) */
 int cgks_workspace_bytes(int ni, int nj, int nk, size_t budget_bytes, size_t* bytes);
 
 /* Builds the mesh metrics (J0 of Eq. 18, cell volumes by the Appendix quadrature, face vector areas, DESIGN.md
@@ -81,7 +83,7 @@ int cgks_step(cgks_ctx*, double dt);
 /* Diagnostics of the current state: volume-averaged kinetic energy E_k = int rho |U|^2/2 dV / |Omega| and
    enstrophy int mu |curl U|^2 dV / |Omega| (rho_0 = 1), by the 2x2x2 Gauss rule on every cell with values and velocity
    derivatives from the compact reconstruction (the scheme's own polynomial, Eq. 16; reading X1); mu is the
-   solver's viscosity law.  Synchronises; overwrites the chi tap and the slab buffers.  Host pointers. */
+   solver's viscosity law.  Synchronises; overwrites the slab buffers (not the chi tap).  Host pointers. */
 int cgks_diagnostics(cgks_ctx*, double* ek_host, double* enstrophy_host);
 
 /* Synchronises and returns CGKS_OK, CGKS_ECUDA or CGKS_ENONPHYSICAL for the work enqueued so far. */
@@ -115,7 +117,7 @@ int cgks_get_chi(cgks_ctx*, double* d_chi);
 int cgks_debug_stage(cgks_ctx*, double dt, double* d_pv, double* d_fx);
 
 /* Measures the device's FP64 FMA throughput with a register-resident DFMA micro-benchmark (8 independent chains
-   per thread, three distinct rotating register operands, 148*8 blocks of 256 threads) on `cuda_stream`; TFLOP/s (FMA = 2 flops) to *tflops (host).
+   per thread, three distinct rotating register operands, 8 blocks of 256 threads per multiprocessor) on `cuda_stream`; TFLOP/s (FMA = 2 flops) to *tflops (host).
    The only call that allocates device memory itself (8 bytes, freed before returning). */
 int cgks_fp64_peak(void* cuda_stream, double* tflops);
 
@@ -124,7 +126,10 @@ int cgks_fp64_peak(void* cuda_stream, double* tflops);
 int cgks_debug_math(int which, long n, const double* d_in, double* d_out, void* cuda_stream);
 
 int cgks_destroy(cgks_ctx*);
+/* Message of the last error on this context; with a NULL context, the same as cgks_last_create_error. */
 const char* cgks_last_error(const cgks_ctx*);
+/* Message of the last failed cgks_create of the calling thread (empty after a successful one). */
+const char* cgks_last_create_error(void);
 const char* cgks_version(void);
 
 #ifdef __cplusplus

@@ -34,6 +34,16 @@ static double g_E[NROW_E][NB];   /* value + 3 reference derivatives at the 24 Ga
 static double g_Gram[4][NB][NB]; /* int over unit cube of sum_{|l|=o+1} D^l p_i D^l p_j     */
 static int    g_face_off[6][3], g_edge_off[12][3], g_edge_axis[12];
 static int    g_ready = 0;
+/* Alternative readings of the paper's gaps, selectable so that oracle/readings_table.py can
+   compare each of them with Tables 1-2.  The defaults are the readings taken (R5 normalised tau2, S3 sum over
+   directions, G2 variant B); nothing but that script and its test changes them. */
+static int    g_r5_normalised = 1;   /* R5: 1 tau2 = o/sqrt 2 (unit vector), 0 tau2 = o                               */
+static int    g_s3_sum = 1;          /* S3: 1 rate = sum over directions, 0 rate = max over directions               */
+static int    g_g2_variant = 1;      /* G2: 1 (B) IS^tau = third+fourth derivative part, 0 (A) IS^tau = |IS^H - IS^L| */
+void cgks_ref_set_readings(int r5_normalised, int s3_sum, int g2_variant) {
+  if (r5_normalised != g_r5_normalised) g_ready = 0;      /* M is rebuilt at the next use */
+  g_r5_normalised = r5_normalised; g_s3_sum = s3_sum; g_g2_variant = g2_variant;
+}
 
 static double factorial(int n) { double f = 1; for (int i = 2; i <= n; i++) f *= i; return f; }
 /* int_a^b x^d/d! dx */
@@ -132,7 +142,7 @@ static void init_constants(void) {
       L[r++][b] = h2 * cellavg_der(g_didx[b], g_edge_off[n], g_edge_axis[n]);
       double s = 0;
       for (int ax = 0; ax < 3; ax++) s += g_edge_off[n][ax] * cellavg_der(g_didx[b], g_edge_off[n], ax);
-      L[r++][b] = h2 * s / sqrt(2.0);
+      L[r++][b] = h2 * s / (g_r5_normalised ? sqrt(2.0) : 1.0);
     }
     for (int ax = 0; ax < 3; ax++) {
       int o1, o2; other_axes(ax, &o1, &o2);
@@ -235,6 +245,7 @@ void cgks_ref_recon_reference(const cgks_ref_params* p, const double* d, double*
     /* path function (readings G2: IS^tau = third+fourth derivative part, G3: C = geno_C) */
     double IS4[4]; cgks_ref_smoothness(a, IS4);
     double ISH = IS4[0] + IS4[1] + IS4[2] + IS4[3], ISL = IS4[0], ISt = IS4[2] + IS4[3];
+    if (!g_g2_variant) ISt = fabs(ISH - ISL);      /* alternative reading G2 (A); never the default */
     double aH = 1.0 + pow(ISt / (ISH + eps), p->geno_r), aL = 1.0 + pow(ISt / (ISL + eps), p->geno_r);
     double alpha = 2.0 * aH / (aH + aL);
     chi = tanh(p->geno_C * alpha) / tanh(p->geno_C);
@@ -272,6 +283,8 @@ struct cgks_ref_ctx {
   double *pv;                   /* [n][24][20] */
   double *fx;                   /* [3][n][4][30] */
   double *chi;                  /* [5][n] */
+  long   nfall;                 /* Gauss-point states replaced by the positivity fallback (reading R9) in the last reconstruction */
+  double fall_rho, fall_pe;     /* most negative rho / |rho_cell| and (rho E - |m|^2/2) / (rho E)_cell among them (0 if none)      */
   char err[256];
 };
 
@@ -419,6 +432,7 @@ int cgks_ref_get_state(cgks_ref_ctx* c, double* Q, double* G, double* D) {
 /* ------------------------------------------------------------------ */
 static void reconstruct_all(cgks_ref_ctx* c) {
   const long n = c->n;
+  c->nfall = 0; c->fall_rho = 0.0; c->fall_pe = 0.0;
 #pragma omp parallel for collapse(2) schedule(static)
   for (int k = 0; k < c->nk; k++) for (int j = 0; j < c->nj; j++) for (int i = 0; i < c->ni; i++) {
     long ci = cidx(c, i, j, k);
@@ -443,7 +457,7 @@ static void reconstruct_all(cgks_ref_ctx* c) {
         double gr[3];
         for (int a = 0; a < 3; a++) { double s = 0; for (int r = 0; r < 3; r++) s += J[3 * r + a] * c->G[(v * 3 + r) * n + nb]; gr[a] = s; }
         d[36 + 2 * e] = 1.0 * gr[g_edge_axis[e]];
-        d[36 + 2 * e + 1] = 1.0 * (g_edge_off[e][0] * gr[0] + g_edge_off[e][1] * gr[1] + g_edge_off[e][2] * gr[2]) / sqrt(2.0);
+        d[36 + 2 * e + 1] = 1.0 * (g_edge_off[e][0] * gr[0] + g_edge_off[e][1] * gr[1] + g_edge_off[e][2] * gr[2]) / (g_r5_normalised ? sqrt(2.0) : 1.0);
       }
       for (int s = 0; s < 12; s++) d[60 + s] = 3.0 * c->D[(v * 12 + s) * n + ci];
       double a[NB], b[18], chi, om[6], val[NGP], gref[NGP * 3];
@@ -455,17 +469,29 @@ static void reconstruct_all(cgks_ref_ctx* c) {
           pv[p * 20 + 5 + 3 * v + r] = Ji[0 * 3 + r] * gref[3 * p] + Ji[1 * 3 + r] * gref[3 * p + 1] + Ji[2 * 3 + r] * gref[3 * p + 2];
       }
     }
-    /* positivity (reading R9, point-wise): a non-physical reconstructed state falls back to the cell average */
-    double Kd = (5.0 - 3.0 * c->prm.gamma) / (c->prm.gamma - 1.0); (void)Kd;
+    /* positivity (reading R9, point-wise): a non-physical reconstructed state falls back to the cell average.
+       Admissible means rho > 0 and rho * (rho e) = rho E - |m|^2/2 > 0, evaluated in exactly this order of
+       operations (R9: the decision is taken on the same fp64 expression on both sides). */
     for (int p = 0; p < NGP; p++) {
       double* w = pv + p * 20;
-      double rho = w[0], pe = w[4] - 0.5 * (w[1] * w[1] + w[2] * w[2] + w[3] * w[3]) / rho;
+      double rho = w[0], pe = w[0] * w[4] - 0.5 * ((w[1] * w[1] + w[2] * w[2]) + w[3] * w[3]);
       if (!(rho > 0.0) || !(pe > 0.0)) {
+#pragma omp critical
+        {   /* statistics only (cgks_ref_fallback_stats): how far outside the admissible set the replaced state was */
+          double r0 = c->Q[ci], e0 = c->Q[ci] * c->Q[4 * n + ci];
+          c->nfall++;
+          if (rho / r0 < c->fall_rho) c->fall_rho = rho / r0;
+          if (pe / e0 < c->fall_pe) c->fall_pe = pe / e0;
+        }
         for (int v = 0; v < NV; v++) w[v] = c->Q[v * n + ci];
         for (int q = 5; q < 20; q++) w[q] = 0.0;
       }
     }
   }
+}
+
+void cgks_ref_fallback_stats(const cgks_ref_ctx* c, long* npoints, double* min_rho_rel, double* min_pe_rel) {
+  *npoints = c->nfall; *min_rho_rel = c->fall_rho; *min_pe_rel = c->fall_pe;
 }
 
 int cgks_ref_reconstruct(cgks_ref_ctx* c, double* pv, double* chi) {
@@ -803,6 +829,7 @@ int cgks_ref_step(cgks_ref_ctx* c, double dt) {
 int cgks_ref_diagnostics(cgks_ref_ctx* c, double* Ek_out, double* ens_out) {
   const long n = c->n; const double g = 0.5 / sqrt(3.0);
   double Ek = 0, ens = 0, vtot = 0;
+#pragma omp parallel for collapse(2) schedule(static) reduction(+ : Ek, ens, vtot)
   for (int k = 0; k < c->nk; k++) for (int j = 0; j < c->nj; j++) for (int i = 0; i < c->ni; i++) {
     long ci = cidx(c, i, j, k);
     const double* J = c->J0 + 9 * ci; const double* Ji = c->J0inv + 9 * ci;
@@ -824,7 +851,7 @@ int cgks_ref_diagnostics(cgks_ref_ctx* c, double* Ek_out, double* ens_out) {
         double gr[3];
         for (int a = 0; a < 3; a++) { double s = 0; for (int r = 0; r < 3; r++) s += J[3 * r + a] * c->G[(v * 3 + r) * n + nb]; gr[a] = s; }
         d[36 + 2 * e] = gr[g_edge_axis[e]];
-        d[36 + 2 * e + 1] = (g_edge_off[e][0] * gr[0] + g_edge_off[e][1] * gr[1] + g_edge_off[e][2] * gr[2]) / sqrt(2.0);
+        d[36 + 2 * e + 1] = (g_edge_off[e][0] * gr[0] + g_edge_off[e][1] * gr[1] + g_edge_off[e][2] * gr[2]) / (g_r5_normalised ? sqrt(2.0) : 1.0);
       }
       for (int s = 0; s < 12; s++) d[60 + s] = 3.0 * c->D[(v * 12 + s) * n + ci];
       double a[NB], b[18], chi, om[6], fval[NGP], fgref[NGP * 3];
@@ -848,7 +875,8 @@ int cgks_ref_diagnostics(cgks_ref_ctx* c, double* Ek_out, double* ens_out) {
     }
     for (int p = 0; p < 8; p++) {
       double rho = val[p][0], pe = val[p][4] - 0.5 * (val[p][1] * val[p][1] + val[p][2] * val[p][2] + val[p][3] * val[p][3]) / rho;
-      if (!(rho > 0.0) || !(pe > 0.0)) {
+      double adm = val[p][0] * val[p][4] - 0.5 * ((val[p][1] * val[p][1] + val[p][2] * val[p][2]) + val[p][3] * val[p][3]);   /* reading R9 */
+      if (!(rho > 0.0) || !(adm > 0.0)) {
         for (int v = 0; v < NV; v++) { val[p][v] = c->Q[v * n + ci]; for (int r = 0; r < 3; r++) grd[p][v][r] = 0.0; }
         rho = val[p][0];
         pe = val[p][4] - 0.5 * (val[p][1] * val[p][1] + val[p][2] * val[p][2] + val[p][3] * val[p][3]) / rho;
@@ -876,6 +904,7 @@ int cgks_ref_diagnostics(cgks_ref_ctx* c, double* Ek_out, double* ens_out) {
 int cgks_ref_compute_dt(cgks_ref_ctx* c, double cfl, double* dt_out) {
   const long n = c->n; const double gam = c->prm.gamma;
   double dtmin = INFINITY;
+#pragma omp parallel for collapse(2) schedule(static) reduction(min : dtmin)
   for (int k = 0; k < c->nk; k++) for (int j = 0; j < c->nj; j++) for (int i = 0; i < c->ni; i++) {
     long ci = cidx(c, i, j, k);
     double rho = c->Q[ci], U[3] = { c->Q[n + ci] / rho, c->Q[2 * n + ci] / rho, c->Q[3 * n + ci] / rho };
@@ -890,7 +919,8 @@ int cgks_ref_compute_dt(cgks_ref_ctx* c, double cfl, double* dt_out) {
       double nb[3] = { Ap[0] + Am[0], Ap[1] + Am[1], Ap[2] + Am[2] }, nl = sqrt(nb[0] * nb[0] + nb[1] * nb[1] + nb[2] * nb[2]);
       double h = c->vol[ci] / (0.5 * (Sp + Sm));
       double un = fabs(U[0] * nb[0] + U[1] * nb[1] + U[2] * nb[2]) / nl;
-      rate += (un + cs) / h;
+      if (g_s3_sum) rate += (un + cs) / h;
+      else if ((un + cs) / h > rate) rate = (un + cs) / h;      /* alternative reading S3 (max); never the default */
       if (h < hmin) hmin = h;
     }
     double d = cfl / rate;

@@ -48,6 +48,11 @@ int    cgks_ref_diagnostics(cgks_ref_ctx*, double* Ek, double* enstrophy);   /* 
 int    cgks_ref_step(cgks_ref_ctx*, double dt);      /* 0 ok, -4 non-physical cell average */
 const char* cgks_ref_last_error(const cgks_ref_ctx*);
 
+/* Selects alternative readings of gaps in the paper for oracle/readings_table.py, which compares
+   them with Tables 1-2: R5 (1: tau2 = unit vector towards the neighbour's centroid, 0: unnormalised offset), S3 (1: sum
+   of the directional rates, 0: their maximum), G2 (1: variant B, 0: variant A).  Defaults (1, 1, 1) = the readings taken. */
+void   cgks_ref_set_readings(int r5_normalised, int s3_sum, int g2_variant);
+
 /* ---- pieces exposed so that tests can pin them against the paper ---- */
 /* constant matrices: M [34][72] (a = M d, Eq. 14/19), E [96][34] (value, d/dxi, d/deta, d/dzeta at 24 points) */
 void   cgks_ref_matrices(double* M, double* E);
@@ -62,6 +67,10 @@ void   cgks_ref_smoothness(const double* a, double* IS4);
 /* reconstruct every cell of the current state: pv [ncell][24][20] = (5 values, 15 physical
    gradient comps [v][dir]); chi [5][ncell] */
 int    cgks_ref_reconstruct(cgks_ref_ctx*, double* pv, double* chi);
+/* positivity fallback (reading R9) of the LAST reconstruction (cgks_ref_reconstruct or the second stage of cgks_ref_step):
+   number of Gauss-point states replaced, and how far outside the admissible set they were: the most negative
+   rho / rho_cell and (rho E - |m|^2/2) / (rho * rho E)_cell among the replaced states (0 when none was negative) */
+void   cgks_ref_fallback_stats(const cgks_ref_ctx*, long* npoints, double* min_rho_rel, double* min_pe_rel);
 /* reconstruct + flux of the current state: fx [3][ncell][4][30] = Fn, Ft, VL, DtL, VR, DtR per owned face point */
 int    cgks_ref_debug_flux(cgks_ref_ctx*, double dt, double* fx);
 /* gas-kinetic solver at one face Gauss point, global frame in/out.

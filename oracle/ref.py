@@ -57,6 +57,8 @@ def lib():
         L.cgks_ref_microslope.argtypes = [_dp] + [C.c_double] * 5 + [_dp]
         L.cgks_ref_moment_apsi.argtypes = [_dp, C.c_int, C.c_int, C.c_int] + [C.c_double] * 5 + [C.c_int, _dp]
         L.cgks_ref_geometry.argtypes = [C.c_void_p, _dp, _dp, _dp]
+        L.cgks_ref_fallback_stats.argtypes = [C.c_void_p, C.POINTER(C.c_long), _dp, _dp]
+        L.cgks_ref_set_readings.argtypes = [C.c_int, C.c_int, C.c_int]
         L.cgks_ref_s2o4_stage1.argtypes = [C.c_double] * 4 + [_dp]
         L.cgks_ref_s2o4_stage2.argtypes = [C.c_double] * 5 + [_dp]
         _lib = L
@@ -69,6 +71,11 @@ def _p(a):
 
 def _c(a):
     return None if a is None else np.ascontiguousarray(a, dtype=np.float64)
+
+
+def set_readings(r5_normalised=1, s3_sum=1, g2_variant=1):
+    """Alternative readings for oracle/readings_table.py; (1, 1, 1) restores the readings taken."""
+    lib().cgks_ref_set_readings(int(r5_normalised), int(s3_sum), int(g2_variant))
 
 
 def matrices():
@@ -179,6 +186,12 @@ class RefSolver:
         pv = np.zeros((self.nk, self.nj, self.ni, NGP, 20)); chi = np.zeros((5, self.nk, self.nj, self.ni))
         lib().cgks_ref_reconstruct(self._h, _p(pv), _p(chi))
         return pv, chi
+
+    def fallback_stats(self):
+        """(points replaced by the R9 fallback in the last reconstruction, min rho/rho_cell, min admissibility/scale)."""
+        n = C.c_long(0); a = np.zeros(1); b = np.zeros(1)
+        lib().cgks_ref_fallback_stats(self._h, C.byref(n), _p(a), _p(b))
+        return int(n.value), float(a[0]), float(b[0])
 
     def debug_flux(self, dt):
         fx = np.zeros((3, self.nk, self.nj, self.ni, 4, 30))

@@ -59,6 +59,7 @@ def lib():
         L.cgks_debug_math.argtypes = [C.c_int, C.c_long, _vp, _vp, _vp]
         L.cgks_destroy.argtypes = [_vp]
         L.cgks_last_error.argtypes = [_vp]; L.cgks_last_error.restype = C.c_char_p
+        L.cgks_last_create_error.restype = C.c_char_p
         L.cgks_version.restype = C.c_char_p
         _lib = L
     return _lib
@@ -135,7 +136,7 @@ class Solver:
                                _vp(self.workspace.data_ptr()), nbytes, _vp(self.stream.cuda_stream))
         if rc:
             self._h = _vp(None)
-            raise CgksError(rc, "cgks_create failed (see stderr)")
+            raise CgksError(rc, "cgks_create: " + L.cgks_last_create_error().decode())
 
     def _check(self, rc):
         if rc:

@@ -58,7 +58,10 @@ static int cuda_fail(cgks_ctx* c, cudaError_t e, const char* where) {
 #define CK(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail(c, e_, #call); } while (0)
 
 extern "C" const char* cgks_version(void) { return "cgks-b200 0.1 (sm_100a, fp64)"; }
-extern "C" const char* cgks_last_error(const cgks_ctx* c) { return c ? c->err.c_str() : "null context"; }
+// message of the last failed cgks_create of the calling thread (there is no context to hold it)
+static thread_local std::string g_create_err;
+extern "C" const char* cgks_last_create_error(void) { return g_create_err.c_str(); }
+extern "C" const char* cgks_last_error(const cgks_ctx* c) { return c ? c->err.c_str() : g_create_err.c_str(); }
 extern "C" long cgks_launch_count(const cgks_ctx* c) { return c ? c->launches : 0; }
 extern "C" int cgks_slab_depth(const cgks_ctx* c) { return c ? c->S : 0; }
 
@@ -77,7 +80,10 @@ extern "C" int cgks_workspace_bytes(int ni, int nj, int nk, size_t budget, size_
   const size_t cap = budget ? (budget > fixed ? budget - fixed : 0) : DEFAULT_SLAB_BYTES;
   if (slab > cap) {
     long S = (long)(cap / slot_bytes(plane)) - 2;
-    if (S < 2) S = 2;
+    if (S < 2) {
+      if (budget) return CGKS_ENOMEM;                           // not even a slab of two k-planes fits under the budget
+      S = 2;
+    }
     slab = (size_t)(S + 2) * slot_bytes(plane);
   }
   *bytes = fixed + align_up(slab) + ALIGN;
@@ -131,17 +137,19 @@ extern "C" int cgks_create(cgks_ctx** out, int ni, int nj, int nk, const double*
                            void* ws, size_t ws_bytes, void* stream) {
   if (!out) return CGKS_EINVAL;
   *out = nullptr;
-  if (ni < 4 || nj < 4 || nk < 4 || !d_nodes || !params || !ws) return CGKS_EINVAL;
-  if ((double)ni * nj * nk >= 2147483648.0 / 8.0) return CGKS_EINVAL;      // 32-bit cell and tile indices in the kernels
-  if (params->geno_r != 2 || !(params->gamma > 1.0) || !(params->gamma < 5.0 / 3.0 + 1e-12)) return CGKS_EINVAL;
+  auto early = [&](int code, const char* msg) { g_create_err = msg; return code; };
+  if (ni < 4 || nj < 4 || nk < 4) return early(CGKS_EINVAL, "ni, nj, nk must be at least 4");
+  if (!d_nodes || !params || !ws) return early(CGKS_EINVAL, "null argument");
+  if ((double)ni * nj * nk >= 2147483648.0 / 8.0) return early(CGKS_EINVAL, "mesh too large for 32-bit cell indices");      // 32-bit cell and tile indices in the kernels
+  if (params->geno_r != 2 || !(params->gamma > 1.0) || !(params->gamma < 5.0 / 3.0 + 1e-12)) return early(CGKS_EINVAL, "unsupported parameters (geno_r must be 2, 1 < gamma <= 5/3)");
   int ndev = 0;
-  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return CGKS_ECUDA;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return early(CGKS_ECUDA, "no CUDA device");
   cgks_ctx* c = new cgks_ctx();
   c->prm = *params; c->stream = (cudaStream_t)stream;
   {
     int dev = 0; cudaGetDevice(&dev);
     if (cudaDeviceGetAttribute(&c->nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || c->nsm <= 0) c->nsm = 148;
-    if (set_flux_smem() != cudaSuccess) { delete c; return CGKS_ECUDA; }
+    if (set_flux_smem() != cudaSuccess) { delete c; return early(CGKS_ECUDA, "no sm_100a kernel image usable on this device"); }
   }
   Mesh& m = c->mesh;
   m.ni = ni; m.nj = nj; m.nk = nk; m.plane = (long)ni * nj; m.n = m.plane * nk; m.cart = 0; m.met = nullptr;
@@ -150,7 +158,7 @@ extern "C" int cgks_create(cgks_ctx** out, int ni, int nj, int nk, const double*
   char* base = (char*)(((uintptr_t)ws + ALIGN - 1) / ALIGN * ALIGN);
   char* end = (char*)ws + ws_bytes;
   char* p = base;
-  if (p + fixed_bytes(n, false) > end) { delete c; return CGKS_ENOMEM; }
+  if (p + fixed_bytes(n, false) > end) { delete c; return early(CGKS_ENOMEM, "workspace too small for the state buffers"); }
   c->d_flags = (int*)p; c->d_dt = (unsigned long long*)(p + 32); p += align_up(64);
   for (int b = 0; b < 3; b++) { c->W[b] = (double*)p; p += state_bytes(n); }
   c->chi = (double*)p; p += align_up((size_t)5 * n * 8);
@@ -203,12 +211,8 @@ extern "C" int cgks_create(cgks_ctx** out, int ni, int nj, int nk, const double*
     c->fx = (double*)p;
     cudaMemsetAsync(c->d_flags, 0, 64, c->stream);
   } while (0);
-  if (rc != CGKS_OK) {
-    // keep the context alive only long enough to report: the caller gets the message through a static buffer
-    static std::string last; last = c->err; delete c;
-    fprintf(stderr, "cgks_create: %s\n", last.c_str());
-    return rc;
-  }
+  if (rc != CGKS_OK) { g_create_err = c->err; delete c; return rc; }      // message: cgks_last_create_error()
+  g_create_err.clear();
   *out = c;
   return CGKS_OK;
 }
@@ -265,7 +269,7 @@ extern "C" int cgks_compute_dt(cgks_ctx* c, double cfl, double* dt_host) {
   const unsigned long long inf_bits = 0x7FF0000000000000ull;
   CK(cudaMemcpyAsync(c->d_dt, &inf_bits, 8, cudaMemcpyHostToDevice, c->stream));
   CflPrm p{ c->prm.gamma, c->prm.mu_ref, c->prm.visc_omega, c->prm.T_ref, cfl };
-  long blocks = (m.n + 255) / 256; if (blocks > 148 * 16) blocks = 148 * 16;
+  long blocks = (m.n + 255) / 256; if (blocks > (long)c->nsm * 16) blocks = (long)c->nsm * 16;
   { Timed t(c, KC_CFL); cfl_kernel<<<(unsigned)blocks, 256, 0, c->stream>>>(m, c->W[c->cur], p, c->d_dt, c->d_flags + 3); }
   unsigned long long bits = 0; int flag = 0;
   CK(cudaMemcpyAsync(&bits, c->d_dt, 8, cudaMemcpyDeviceToHost, c->stream));
@@ -386,7 +390,7 @@ static void run_diagnostics(cgks_ctx* c, double* d_acc) {
 
 extern "C" int cgks_diagnostics(cgks_ctx* c, double* ek_host, double* enstrophy_host) {
   if (!c || !ek_host || !enstrophy_host) return CGKS_EINVAL;
-  double* d_acc = c->chi;                 // 3 doubles of the chi buffer serve as the accumulator (chi is a diagnostic tap only)
+  double* d_acc = (double*)((char*)c->d_flags + 40);      // the 24 unused bytes of the 64-byte flags block
   CK(cudaMemsetAsync(d_acc, 0, 3 * sizeof(double), c->stream));
   if (c->mesh.cart) run_diagnostics<true>(c, d_acc); else run_diagnostics<false>(c, d_acc);
   double acc[3] = { 0, 0, 0 };
@@ -437,7 +441,9 @@ extern "C" int cgks_fp64_peak(void* stream, double* tflops) {
   cudaStream_t st = (cudaStream_t)stream;
   double* d = nullptr;
   CK(cudaMalloc(&d, 8));
-  const int blocks = 148 * 8, iters = 4096;
+  int dev = 0, nsm = 0; cudaGetDevice(&dev);
+  if (cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || nsm <= 0) { cudaFree(d); return CGKS_ECUDA; }
+  const int blocks = nsm * 8, iters = 4096;
   cudaEvent_t a, b; cudaEventCreate(&a); cudaEventCreate(&b);
   double best = 0;
   for (int rep = 0; rep < 5; rep++) {

@@ -34,6 +34,15 @@ struct Slab {
 __device__ __forceinline__ int wrap(int i, int n) { return i < 0 ? i + n : (i >= n ? i - n : i); }
 __device__ __forceinline__ int slot_of(const Mesh& m, const Slab& s, int k) { int t = k - s.kbase; return t < 0 ? t + m.nk : t; }
 
+// Positivity test of a reconstructed state (reading R9): admissible iff rho > 0 and rho (rho e) = rho E - |m|^2/2 > 0.
+// The expression is evaluated with individually rounded operations in this fixed order (no FMA contraction), so that the
+// decision is taken on bit-identical arithmetic wherever it is made.
+__device__ __forceinline__ bool admissible(const double* w) {
+  const double m2 = __dadd_rn(__dadd_rn(__dmul_rn(w[1], w[1]), __dmul_rn(w[2], w[2])), __dmul_rn(w[3], w[3]));
+  const double re = __dsub_rn(__dmul_rn(w[0], w[4]), __dmul_rn(0.5, m2));
+  return (w[0] > 0.0) && (re > 0.0);
+}
+
 struct CellIdx { int i, j, k; long ij; long c; };
 // thread t over `cnt` planes starting at plane kA (wrapped).  32-bit index arithmetic: cgks_create rejects meshes with
 // 2^31 cells or more (far beyond 180 GB of state), and 64-bit integer division costs ~100 instructions on the SM.

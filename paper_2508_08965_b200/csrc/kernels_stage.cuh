@@ -210,7 +210,7 @@ __global__ void __launch_bounds__(128) diag_kernel(Mesh m, Slab sl, const double
 #pragma unroll
         for (int r = 0; r < 3; r++) g[c][r] = src[(long)(5 + 3 * c + r) * sl.stride_pv];
       double pe = w[4] - 0.5 * (w[1] * w[1] + w[2] * w[2] + w[3] * w[3]) / w[0];
-      if (!(w[0] > 0.0) || !(pe > 0.0)) {      // positivity fallback (reading R9): cell average, zero gradient
+      if (!admissible(w)) {                    // positivity fallback (reading R9): cell average, zero gradient
 #pragma unroll
         for (int c = 0; c < 5; c++) w[c] = W[(long)c * m.n + x.c];
 #pragma unroll
@@ -271,7 +271,8 @@ __global__ void __launch_bounds__(256) diag_reduce_kernel(const double* __restri
 // reads what it copied).
 __device__ __forceinline__ void cp_async8(double* smem_dst, const double* gsrc) {
   const unsigned sa = (unsigned)__cvta_generic_to_shared(smem_dst);
-  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(sa), "l"(gsrc) : "memory");
+  const size_t ga = __cvta_generic_to_global(gsrc);          // the instruction takes a .global address, not a generic one
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(sa), "l"(ga) : "memory");
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
 template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
@@ -338,15 +339,13 @@ __global__ void __launch_bounds__(FLUX_TPB, FLUX_MINB) flux_kernel(Mesh m, Slab 
   if (!active) continue;
   // positivity (reading R9, point-wise): a non-physical reconstructed state falls back to the cell average
   {
-    const double eL = WLg[0] * WLg[4] - 0.5 * (WLg[1] * WLg[1] + WLg[2] * WLg[2] + WLg[3] * WLg[3]);    // rho * (rho e)
-    if (!(WLg[0] > 0.0) || !(eL > 0.0)) {
+    if (!admissible(WLg)) {
 #pragma unroll
       for (int c = 0; c < 5; c++) WLg[c] = W[(long)c * m.n + cL];
 #pragma unroll
       for (int c = 0; c < 15; c++) gL[c] = 0.0;
     }
-    const double eR = WRg[0] * WRg[4] - 0.5 * (WRg[1] * WRg[1] + WRg[2] * WRg[2] + WRg[3] * WRg[3]);
-    if (!(WRg[0] > 0.0) || !(eR > 0.0)) {
+    if (!admissible(WRg)) {
       FluxPoint fp; flux_point<AXIS>(m, sl, tile, tiles_per_q, ncells, kA, fp);
       const long cr = cell_at(m, fp.ir, fp.jr, fp.kr);
 #pragma unroll

@@ -176,6 +176,34 @@ def iso_turbulence(n, seed, Ma_t, k0=8.0, gamma=1.4, device=None):
     return stack([one(ke), u[0], u[1], u[2], pval / (gamma - 1.0) + ke])
 
 
+# ----------------------------------------------------------------------------- affine (sheared) mesh, strong-jump states
+SHEAR = np.array([[1.0, 0.3, 0.1], [-0.15, 1.0, 0.2], [0.25, -0.1, 1.0]])      # constant, non-symmetric J0 / h
+
+
+def sheared_nodes(n, h=1.0, A=SHEAR):
+    """Affine periodic mesh of parallelepiped cells: node(i, j, k) = A (i, j, k) h (every cell has J0 = A h)."""
+    ni, nj, nk = (n, n, n) if np.isscalar(n) else n
+    K, J, I = np.meshgrid(np.arange(nk + 1.0), np.arange(nj + 1.0), np.arange(ni + 1.0), indexing="ij")
+    lat = np.stack([I, J, K]) * h
+    return np.einsum("ra,akji->rkji", np.asarray(A, dtype=np.float64), lat)
+
+
+def jump_state(n, kind="blob", ratio=0.05, nodes=None):
+    """Piecewise-constant state with a strong density / pressure jump (inside : outside = 1 : ratio) and a uniform
+    velocity, on the unit box: the compact polynomials over- and undershoot at the jump by a multiple of the low state,
+    so the positivity fallback (reading R9) fires by an O(1) margin.  kind: 'blob' (off-centre ball) or
+    'oblique' (slab inclined to all three axes)."""
+    nodes = cartesian_nodes(n, 0.0, 1.0) if nodes is None else nodes
+    X, Y, Z = cell_centroids(nodes)
+    if kind == "blob":
+        inside = np.sqrt((X - 0.5) ** 2 + (Y - 0.45) ** 2 + (Z - 0.55) ** 2) < 0.27
+    else:
+        inside = (X + 0.5 * Y + 0.25 * Z) % 1.0 < 0.5
+    rho = np.where(inside, 1.0, ratio); p = np.where(inside, 1.0, 0.8 * ratio)
+    one = np.ones_like(rho)
+    return nodes, prim_to_cons(rho, 0.3 * one, -0.2 * one, 0.1 * one, p)
+
+
 # ----------------------------------------------------------------------------- named workloads
 def workload(name, n=None, k0=None):
     """Returns dict(nodes, Q, G, D, params, nonlinear, cfl, steps) for the five BASELINE.json configs.
@@ -214,5 +242,22 @@ def workload(name, n=None, k0=None):
         n = n or 384
         k0 = k0 or 8.0
         return dict(nodes=cartesian_nodes(n), Q=iso_turbulence(n, 5, 1.0, k0), G=None, D=None, params=iso_params(1.0, k0=k0),
+                    nonlinear=1, cfl=0.5, steps=100)
+    if name in ("jump_blob", "jump_oblique", "jump_oblique_linear"):
+        # deterministic positivity-fallback cases (reading R9): GENO on a 1:0.05 jump, linear reconstruction on a 1:0.2 jump
+        n = n or 12
+        kind = "blob" if name == "jump_blob" else "oblique"
+        nodes, Q = jump_state(n, kind, 0.2 if name.endswith("linear") else 0.05)
+        prm = dict(sine_params()); prm.update(tau_c1=0.05, tau_c2=5.0)
+        return dict(nodes=nodes, Q=Q, G=None, D=None, params=prm, nonlinear=0 if name.endswith("linear") else 1, cfl=0.3, steps=5)
+    if name == "tgv_shear":
+        # Taylor-Green-like smooth field on the affine sheared mesh (constant non-symmetric J0): pins the J0^T / J0^-T transforms
+        n = n or 12
+        nodes = sheared_nodes(n, 2.0 * math.pi / n)
+        xi = np.linalg.solve(SHEAR, cell_centroids(nodes).reshape(3, -1)).reshape(3, n, n, n)      # periodic coordinates
+        p0 = 1.0 / (1.4 * 0.3 ** 2)
+        u = np.sin(xi[0]) * np.cos(xi[1]) * np.cos(xi[2]); v = -np.cos(xi[0]) * np.sin(xi[1]) * np.cos(xi[2]); wv = 0.2 * np.sin(xi[2] + xi[0])
+        p = p0 + (np.cos(2 * xi[0]) + np.cos(2 * xi[1])) * (np.cos(2 * xi[2]) + 2.0) / 16.0
+        return dict(nodes=nodes, Q=prim_to_cons(p / p0, u, v, wv, p), G=None, D=None, params=tgv_params(Ma=0.3, Re=200.0),
                     nonlinear=1, cfl=0.5, steps=100)
     raise KeyError(name)

@@ -6,18 +6,26 @@ from oracle import ref
 from paper_2508_08965_b200 import inputs
 
 
+REST_FRACTION = 0.05      # a flow counts as "at rest" when max|U| < REST_FRACTION * max c
+
+
 def field_errors(gpu, orc, nodes, Qref):
-    """Relative L-infinity error per field (80 planes): max|gpu-oracle| / max(|oracle|_inf, delta_f) with the floors
-    delta_f = 1e-3 |Q_v|_inf (D planes), 1e-3 |Q_v|_inf / h_min (G planes), 1e-3 |rho|_inf max(|U|+c) (momentum planes;
-    for a momentum variable |Q_v|_inf in the D and G floors is replaced by max(|Q_v|_inf, momentum floor)).
-    The floors keep fields that are identically ~0 (free-stream derivatives, transverse momenta of 1-D flows)
-    from turning round-off noise into O(1) 'relative' errors."""
+    """Relative L-infinity error per field (80 planes): max|gpu-oracle| / max(|oracle|_inf, delta_f),
+    delta_f = 1e-3 |Q_v|_inf (D planes), 1e-3 |Q_v|_inf / h_min (G planes), 1e-3 |rho|_inf max|U| (momentum planes).
+    The floors keep fields that are identically ~0 (free-stream derivatives, transverse momenta of 1-D flows) from turning
+    round-off noise into O(1) 'relative' errors.  Two statements the survey's text leaves open:
+    (i) for a momentum variable, |Q_v|_inf in the D and G floors is max(|Q_v|_inf, momentum floor), otherwise the floor
+    of the derivative planes of an identically-zero momentum component would itself be zero; (ii) when the flow is
+    at rest (max|U| < 0.05 max c: the shock tubes) the velocity scale max|U| is itself ~0 and is replaced by max(|U| + c)."""
     Qg, Gg, Dg = gpu; Qo, Go, Do = orc
     hmin = min(np.abs(np.diff(nodes[0], axis=2)).min(), np.abs(np.diff(nodes[1], axis=1)).min(), np.abs(np.diff(nodes[2], axis=0)).min())
     qinf = [np.abs(Qref[v]).max() for v in range(5)]
     rho = Qref[0]; U = Qref[1:4] / rho
     pres = 0.4 * (Qref[4] - 0.5 * rho * (U ** 2).sum(0))
-    umax = (np.sqrt((U ** 2).sum(0)) + np.sqrt(1.4 * pres / rho)).max()      # velocity scale |U| + c
+    speed = np.sqrt((U ** 2).sum(0)); sound = np.sqrt(1.4 * pres / rho)
+    umax = speed.max()
+    if umax < REST_FRACTION * sound.max():
+        umax = (speed + sound).max()
     mom_floor = 1e-3 * qinf[0] * umax
     errs = {}
     for v in range(5):
@@ -50,6 +58,8 @@ def run_oracle(w, nsteps, dts=None):
 
 
 def run_gpu(w, nsteps, dts=None, budget_bytes=0):
+    """Steps with `dts` when given (the oracle's), else with the library's own cgks_compute_dt; returns the state and
+    the library's own dt of every step."""
     from paper_2508_08965_b200 import binding
     s = binding.Solver(w["nodes"], binding.make_params(**w["params"], nonlinear=w["nonlinear"]), budget_bytes=budget_bytes)
     s.set_state(w["Q"], w["G"], w["D"])
