@@ -9,14 +9,21 @@ from paper_2508_08965_b200 import inputs
 REST_FRACTION = 0.05      # a flow counts as "at rest" when max|U| < REST_FRACTION * max c
 
 
-def field_errors(gpu, orc, nodes, Qref):
+def field_errors(gpu, orc, nodes, Qref, mask=None):
     """Relative L-infinity error per field (80 planes): max|gpu-oracle| / max(|oracle|_inf, delta_f),
     delta_f = 1e-3 |Q_v|_inf (D planes), 1e-3 |Q_v|_inf / h_min (G planes), 1e-3 |rho|_inf max|U| (momentum planes).
     The floors keep fields that are identically ~0 (free-stream derivatives, transverse momenta of 1-D flows) from turning
     round-off noise into O(1) 'relative' errors.  Two statements the survey's text leaves open:
     (i) for a momentum variable, |Q_v|_inf in the D and G floors is max(|Q_v|_inf, momentum floor), otherwise the floor
     of the derivative planes of an identically-zero momentum component would itself be zero; (ii) when the flow is
-    at rest (max|U| < 0.05 max c: the shock tubes) the velocity scale max|U| is itself ~0 and is replaced by max(|U| + c)."""
+    at rest (max|U| < 0.05 max c: the shock tubes) the velocity scale max|U| is itself ~0 and is replaced by max(|U| + c).
+    `mask` (bool, cells) restricts the numerators to the cells it selects (the scales stay those of the whole field)."""
+    sel = (lambda a: a) if mask is None else (lambda a: a[mask])
+    return {k: sel(e).max() for k, e in element_errors(gpu, orc, nodes, Qref).items()}
+
+
+def element_errors(gpu, orc, nodes, Qref):
+    """|gpu - oracle| of every element divided by the field's scale max(|oracle_f|_inf, delta_f) (see field_errors)."""
     Qg, Gg, Dg = gpu; Qo, Go, Do = orc
     hmin = min(np.abs(np.diff(nodes[0], axis=2)).min(), np.abs(np.diff(nodes[1], axis=1)).min(), np.abs(np.diff(nodes[2], axis=0)).min())
     qinf = [np.abs(Qref[v]).max() for v in range(5)]
@@ -31,11 +38,11 @@ def field_errors(gpu, orc, nodes, Qref):
     for v in range(5):
         floor = mom_floor if 1 <= v <= 3 else 0.0
         qfloor = max(qinf[v], mom_floor) if 1 <= v <= 3 else qinf[v]
-        errs["Q%d" % v] = np.abs(Qg[v] - Qo[v]).max() / max(np.abs(Qo[v]).max(), floor, 1e-300)
+        errs["Q%d" % v] = np.abs(Qg[v] - Qo[v]) / max(np.abs(Qo[v]).max(), floor, 1e-300)
         for r in range(3):
-            errs["G%d_%d" % (v, r)] = np.abs(Gg[v, r] - Go[v, r]).max() / max(np.abs(Go[v, r]).max(), 1e-3 * qfloor / hmin)
+            errs["G%d_%d" % (v, r)] = np.abs(Gg[v, r] - Go[v, r]) / max(np.abs(Go[v, r]).max(), 1e-3 * qfloor / hmin)
         for s in range(12):
-            errs["D%d_%d" % (v, s)] = np.abs(Dg[v, s] - Do[v, s]).max() / max(np.abs(Do[v, s]).max(), 1e-3 * qfloor)
+            errs["D%d_%d" % (v, s)] = np.abs(Dg[v, s] - Do[v, s]) / max(np.abs(Do[v, s]).max(), 1e-3 * qfloor)
     return errs
 
 

@@ -84,11 +84,47 @@ def test_positivity_fallback_parity(name):
 
 def test_rough_field_one_step_parity_and_robustness():
     """Badly under-resolved Ma_t = 1 field (16^3, k0 = 8; the case VERDICT r1 item 3 names): the fallback (reading R9)
-    fires on near-vacuum states.  One step is compared with the oracle element by element; after that the run must stay
-    physical and conservative (element-wise parity over many steps of an under-resolved shocked field measures the
-    growth of round-off in both codes, not an implementation difference: see test_restart_parity for the multi-step check)."""
+    fires, and some ADMITTED Gauss-point states are near vacuum (internal energy 8e-6 of the total energy), where the
+    kinetic flux has a condition number of ~1e6.  Checked: (i) both sides replace exactly the same points; (ii) the
+    reconstructed values agree to 1e-13 everywhere; (iii) after one step every element agrees to 1e-10 wherever the
+    ORACLE ITSELF is well conditioned, i.e. where a 2-ulp relative perturbation of its input moves its own result by less
+    than 1e-12 (> 95 % of the elements), and within 200 x the oracle's own sensitivity elsewhere; then the run must stay
+    physical and conservative."""
+    from oracle import ref
+    from paper_2508_08965_b200 import binding
     w = parity.build_case("iso_sup", 16, 1)
-    _check(w, 1, TOL_1)
+    so = ref.RefSolver(w["nodes"], ref.make_params(**w["params"], nonlinear=1)); so.set_state(w["Q"])
+    pvo, _ = so.reconstruct()
+    nfall = so.fallback_stats()[0]
+    so.close()
+    s = binding.Solver(w["nodes"], binding.make_params(**w["params"], nonlinear=1)); s.set_state(w["Q"])
+    pv, _ = s.debug_stage()
+    s.close()
+    pvg = np.moveaxis(pv.cpu().numpy(), (0, 1), (3, 4))
+    adm = pvg[..., 0] * pvg[..., 4] - 0.5 * ((pvg[..., 1] * pvg[..., 1] + pvg[..., 2] * pvg[..., 2]) + pvg[..., 3] * pvg[..., 3])
+    bad_g = ~((pvg[..., 0] > 0) & (adm > 0))
+    Qc = np.moveaxis(w["Q"], 0, -1)[:, :, :, None, :]
+    flat_o = (np.abs(pvo[..., 5:]).max(-1) == 0) & (np.abs(pvo[..., :5] - Qc).max(-1) == 0)
+    assert nfall > 0 and bad_g.sum() == nfall and np.array_equal(bad_g, flat_o)
+    assert np.abs(pvg - pvo)[~bad_g].max() < 1e-13 * np.abs(pvo).max()
+    assert ((adm / (Qc[..., 0] * Qc[..., 4]) < 1e-4) & ~bad_g).any()           # a near-vacuum state is admitted
+    orc, dts = parity.run_oracle(w, 1)
+    gpu, dts_gpu = parity.run_gpu(w, 1, dts=dts)
+    assert abs(dts_gpu[0] / dts[0] - 1) <= 1e-13
+    err = parity.element_errors(gpu, orc, w["nodes"], w["Q"])
+    sens = None
+    for seed in (1, 2):
+        w2 = dict(w); w2["Q"] = w["Q"] * (1.0 + 4.4e-16 * np.random.default_rng(seed).uniform(-1, 1, w["Q"].shape))
+        pert, _ = parity.run_oracle(w2, 1, dts=dts)
+        e2 = parity.element_errors(pert, orc, w["nodes"], w["Q"])
+        sens = e2 if sens is None else {k: np.maximum(sens[k], e2[k]) for k in e2}
+    nwell = ntot = 0
+    for k in err:
+        well = sens[k] < 1e-12
+        nwell += int(well.sum()); ntot += well.size
+        assert err[k][well].max() <= TOL_1, (k, err[k][well].max())
+        assert (err[k][~well] <= 200 * sens[k][~well]).all(), k
+    assert nwell > 0.95 * ntot, (nwell, ntot)
     gpu, _ = parity.run_gpu(w, 50)
     assert np.isfinite(gpu[0]).all() and gpu[0][0].min() > 0
     np.testing.assert_allclose(gpu[0].sum(axis=(1, 2, 3)), w["Q"].sum(axis=(1, 2, 3)), rtol=1e-12, atol=1e-9)
@@ -408,7 +444,6 @@ def _restart_parity(s, nodes, params, nonlinear, lows, B, tol, dt=None, need_chi
     s.step(dt); s.status()
     Q1, G1, D1 = s.get_state()
     worst = 0.0
-    nd = torch.as_tensor(nodes)
     for lo, qb, gb, db in blocks:
         # nodes of the block: B+1 planes per direction starting at lo (the mesh is periodic: wrap with the period vector)
         bn = _block_nodes(nodes, lo, B)
@@ -529,9 +564,12 @@ def test_flux_tap_matches_oracle_per_axis():
         pv, fx = s.debug_stage(dt)
         pv = pv.cpu().numpy(); fx = fx.cpu().numpy(); s.close()
         pvg = np.moveaxis(pv, (0, 1), (3, 4))                      # [24][20][k][j][i] -> [k][j][i][24][20]
+        worst = {}
         for c in range(20):
-            sc = np.abs(pvo[..., c]).max() + 1e-3 * np.abs(pvo[..., c % 5 if c < 5 else (c - 5) // 3]).max() * n
-            assert np.abs(pvg[..., c] - pvo[..., c]).max() <= 1e-11 * sc, (name, "pv", c)
+            var = c if c < 5 else (c - 5) // 3
+            sc = np.abs(pvo[..., c]).max() + 1e-3 * np.abs(pvo[..., var]).max() * n + 1e-300
+            worst["pv"] = max(worst.get("pv", 0.0), np.abs(pvg[..., c] - pvo[..., c]).max() / sc)
+        names = ["Fn", "Ft", "VL", "DtL", "VR", "DtR"]
         for ax in range(3):
             for q in range(4):
                 g = np.moveaxis(fx[4 * ax + q], 0, -1)             # [30][k][j][i] -> [k][j][i][30]
@@ -539,7 +577,14 @@ def test_flux_tap_matches_oracle_per_axis():
                 for grp in range(6):
                     sl = slice(5 * grp, 5 * grp + 5)
                     sc = np.abs(o[..., sl]).max(axis=(0, 1, 2)) + 1e-3 * np.abs(o[..., sl]).max()
-                    assert (np.abs(g[..., sl] - o[..., sl]).max(axis=(0, 1, 2)) <= 2e-10 * sc).all(), (name, ax, q, grp)
+                    e = (np.abs(g[..., sl] - o[..., sl]).max(axis=(0, 1, 2)) / sc).max()
+                    key = "%s ax%d" % (names[grp], ax)
+                    worst[key] = max(worst.get(key, 0.0), e)
+        print(name, {k: "%.1e" % v for k, v in worst.items()})
+        assert worst["pv"] <= 1e-11, worst
+        for k, v in worst.items():
+            if k != "pv":
+                assert v <= (1e-12 if k[:2] in ("Fn", "VL", "VR") else 2e-11), (name, k, v)
 
 
 @pytest.mark.parametrize("pinned", [True, False])

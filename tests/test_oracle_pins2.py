@@ -96,8 +96,9 @@ def test_sheared_mesh_quartic_exactness():
 
 
 def test_one_step_on_the_sheared_mesh_is_frame_consistent():
-    """The same physical flow computed on the sheared mesh and on a Cartesian mesh agrees to the truncation error, which
-    falls with the design order under refinement (a wrong J0 transform gives an O(1) discrepancy that does not fall)."""
+    """One short step of a smooth flow on the sheared mesh: the change of the cell-averaged mass equals -div(rho U), with
+    the divergence evaluated spectrally in the periodic coordinates, up to a truncation error that falls under refinement
+    (a wrong J0 transform gives an O(1) discrepancy that does not fall)."""
     errs = []
     for n in (8, 16):
         w = inputs.workload("tgv_shear", n)
