@@ -5,13 +5,17 @@
 // (Eq. 6-7): F^n, F_t^n, and the one-sided interface values Q^{l,r}, Q_t^{l,r}.
 // Collision time per PAPER.md:344-352.  Readings of the paper's gaps: DESIGN.md section 3 (F1-F3, T1-T2).
 //
-// Formulation (differs from the CPU oracle on purpose).  With psi = (1, u, v, w, (u^2+T2)/2),
-// T2 = v^2 + w^2 + xi^2, every term of Eq. 5 is a moment <(a.psi) u^I v^J w^K psi_alpha> of a Maxwellian.  The
-// tangential velocities and xi are integrated out FIRST with three small tables per Maxwellian
-//     P0[q][r] = <v^q w^r>,  P2[q][r] = <T2 v^q w^r>,  P4[q][r] = <T2^2 v^q w^r>,
-// which leaves, per weight phi in {1, v, w, T2}, a polynomial in u ("UPoly"); the spatial-divergence combination
-// a_x u + a_y v + a_z w of Eq. 5 is summed as ONE cubic per weight before any u-moment is applied, and the same cubic
-// serves the compatibility condition (full u-moments), the conserved moments (shift 0) and the flux moments (shift 1).
+// Formulation (differs from the CPU oracle on purpose).  Every term of Eq. 5 is a moment
+// <(a.psi) u^I v^J w^K psi_alpha> of a Maxwellian, psi = (1, u, v, w, (u^2+v^2+w^2+xi^2)/2).  For each Maxwellian the
+// tangential velocities are measured from its own mean, c_v = v - V, c_w = w - W, T = c_v^2 + c_w^2 + xi^2, and slopes and
+// moments are carried in the basis psi' = (1, u, c_v, c_w, (u^2 + T)/2) ("primed"):
+//     psi = B psi',  B = [1; u; V + c_v; W + c_w; psi'_4 + V c_v + W c_w + (V^2+W^2)/2].
+// In that basis the (c_v, c_w, xi) integrals are the central moments <c_v^2> = 1/(2 lam), <T> = (K+2)/(2 lam), ... so no
+// moment tables are needed: a slope leaves ONE quadratic in u (weight 1) plus two constants (weights c_v, c_w), and the
+// spatial-divergence combination a_x u + a_y v + a_z w of Eq. 5 leaves one cubic and two quadratics.  The micro-slope
+// solve is done directly in the primed basis (its tangential part decouples: a'_2 = 2 lam h'_2), the compatibility
+// condition hands its primed moments straight to the solve of the time slope, and only what is summed over BOTH sides
+// (different V, W) is converted to the laboratory basis, 10 FMAs per moment vector.
 #pragma once
 #include <math.h>
 #include "fastmath64.cuh"
@@ -26,14 +30,13 @@ struct GasConst {
   double c1, c2;       // tau = mu/p + c1 dt + c2 |pl-pr|/|pl+pr| dt
 };
 
-// Maxwellian per unit density with the tangential tables
+// Maxwellian (per unit density) and the constants of its primed basis
 struct Maxw {
   double rho, irho, U, V, W, lam, hil;   // hil = 1/(2 lam) = p/rho
-  double s;                              // U^2+V^2+W^2 + (K+3)/(2 lam)
+  double sU;                             // U^2 + (K+3)/(2 lam)
   double c4;                             // 4 lam^2/(K+3)
-  double P0[4][4];                       // q + r <= 3 used
-  double P2[3][3];                       // q + r <= 2 used
-  double P4[2][2];                       // q + r <= 1 used
+  double q2;                             // (V^2 + W^2)/2
+  double t1;                             // <T> = (K+2)/(2 lam)
 };
 
 // scalars of the Maxwellian of the conservative state Wc.  ONE division: with re = rho E - |m|^2/2 = rho (rho e),
@@ -47,31 +50,10 @@ __device__ __forceinline__ void maxw_scalars(Maxw& g, const double* Wc, const Ga
   g.U = Wc[1] * g.irho; g.V = Wc[2] * g.irho; g.W = Wc[3] * g.irho;
   g.hil = 2.0 * gc.inv_K3 * re * (g.irho * g.irho);          // 1/(2 lam) = 2 (rho e)/((K+3) rho) = p/rho
   g.lam = 0.25 * (gc.K + 3.0) * (Wc[0] * Wc[0]) * ire;
-  const double k3h = (gc.K + 3.0) * g.hil;
-  g.s = g.U * g.U + g.V * g.V + g.W * g.W + k3h;
+  g.sU = fma(g.U, g.U, (gc.K + 3.0) * g.hil);
   g.c4 = 4.0 * g.lam * g.lam * gc.inv_K3;
-}
-
-__device__ __forceinline__ void maxw_tables(Maxw& g, const GasConst& gc) {
-  double mv[6], mw[6];
-  mv[0] = 1.0; mv[1] = g.V; mw[0] = 1.0; mw[1] = g.W;
-#pragma unroll
-  for (int n = 0; n < 4; n++) { mv[n + 2] = g.V * mv[n + 1] + (n + 1) * g.hil * mv[n]; mw[n + 2] = g.W * mw[n + 1] + (n + 1) * g.hil * mw[n]; }
-  const double x2 = gc.K * g.hil, x4 = gc.K * (gc.K + 2.0) * g.hil * g.hil;
-#pragma unroll
-  for (int q = 0; q < 4; q++)
-#pragma unroll
-    for (int r = 0; r + q < 4; r++) g.P0[q][r] = mv[q] * mw[r];
-#pragma unroll
-  for (int q = 0; q < 3; q++)
-#pragma unroll
-    for (int r = 0; r + q < 3; r++) g.P2[q][r] = mv[q + 2] * mw[r] + mv[q] * mw[r + 2] + x2 * g.P0[q][r];
-#pragma unroll
-  for (int q = 0; q < 2; q++)
-#pragma unroll
-    for (int r = 0; r + q < 2; r++)
-      g.P4[q][r] = mv[q + 4] * mw[r] + mv[q] * mw[r + 4] + x4 * g.P0[q][r]
-                 + 2.0 * (mv[q + 2] * mw[r + 2] + x2 * (mv[q + 2] * mw[r] + mv[q] * mw[r + 2]));
+  g.q2 = 0.5 * fma(g.V, g.V, g.W * g.W);
+  g.t1 = (gc.K + 2.0) * g.hil;
 }
 
 // first two half-space moments (times rho) of a Maxwellian: SGN = +1 -> u > 0, -1 -> u < 0
@@ -91,49 +73,44 @@ __device__ __forceinline__ void mom_recur(double* m, double U, double hil) {
   for (int n = 0; n + 2 < N; n++) m[n + 2] = U * m[n + 1] + (n + 1) * hil * m[n];
 }
 
-// solves <(a.psi) psi> = h for the micro slope a (standard GKS relation)
-__device__ __forceinline__ void micro_slope(const Maxw& g, const double* h, double* a) {
-  const double R1 = h[1] - g.U * h[0], R2 = h[2] - g.V * h[0], R3 = h[3] - g.W * h[0];
-  const double R4 = 2.0 * h[4] - g.s * h[0];
+// Micro slope in the primed basis, a = (a'_0, a_1, a'_2, a'_3, a_4) with a.psi = a'.psi', from the PRIMED moments
+// hp[alpha] = <(a.psi) psi'_alpha> per unit density (the standard GKS relation with V = W = 0).
+__device__ __forceinline__ void micro_slope_primed(const Maxw& g, const double* hp, double* a) {
+  const double R1 = hp[1] - g.U * hp[0];
+  const double R4 = 2.0 * hp[4] - g.sU * hp[0];
   const double tl = 2.0 * g.lam;
-  a[4] = g.c4 * (R4 - 2.0 * (g.U * R1 + g.V * R2 + g.W * R3));
+  a[4] = g.c4 * (R4 - 2.0 * (g.U * R1));
   a[1] = tl * R1 - g.U * a[4];
-  a[2] = tl * R2 - g.V * a[4];
-  a[3] = tl * R3 - g.W * a[4];
-  a[0] = h[0] - g.U * a[1] - g.V * a[2] - g.W * a[3] - 0.5 * a[4] * g.s;
+  a[2] = tl * hp[2];
+  a[3] = tl * hp[3];
+  a[0] = hp[0] - g.U * a[1] - 0.5 * (a[4] * g.sU);
 }
 
-// polynomial in u per weight phi = 0:1, 1:v, 2:w, 3:T2 of  <(a.psi) phi v^J w^K>_{v,w,xi} = c[phi][0] + c[phi][1] u + c[phi][2] u^2
-struct UPoly { double c[4][3]; };
-
-template <int J, int Kw>
-__device__ __forceinline__ void make_upoly(UPoly& p, const Maxw& g, const double* a) {
-  const double h4 = 0.5 * a[4];
-  // phi = 1
-  p.c[0][0] = a[0] * g.P0[J][Kw] + a[2] * g.P0[J + 1][Kw] + a[3] * g.P0[J][Kw + 1] + h4 * g.P2[J][Kw];
-  p.c[0][1] = a[1] * g.P0[J][Kw];               p.c[0][2] = h4 * g.P0[J][Kw];
-  // phi = v
-  p.c[1][0] = a[0] * g.P0[J + 1][Kw] + a[2] * g.P0[J + 2][Kw] + a[3] * g.P0[J + 1][Kw + 1] + h4 * g.P2[J + 1][Kw];
-  p.c[1][1] = a[1] * g.P0[J + 1][Kw];           p.c[1][2] = h4 * g.P0[J + 1][Kw];
-  // phi = w
-  p.c[2][0] = a[0] * g.P0[J][Kw + 1] + a[2] * g.P0[J + 1][Kw + 1] + a[3] * g.P0[J][Kw + 2] + h4 * g.P2[J][Kw + 1];
-  p.c[2][1] = a[1] * g.P0[J][Kw + 1];           p.c[2][2] = h4 * g.P0[J][Kw + 1];
-  // phi = T2
-  p.c[3][0] = a[0] * g.P2[J][Kw] + a[2] * g.P2[J + 1][Kw] + a[3] * g.P2[J][Kw + 1] + h4 * g.P4[J][Kw];
-  p.c[3][1] = a[1] * g.P2[J][Kw];               p.c[3][2] = h4 * g.P2[J][Kw];
+// the same from LABORATORY moments h[alpha] = <(a.psi) psi_alpha>: psi' = B^-1 psi first
+__device__ __forceinline__ void micro_slope_lab(const Maxw& g, const double* h, double* a) {
+  double hp[5];
+  hp[0] = h[0]; hp[1] = h[1];
+  hp[2] = h[2] - g.V * h[0];
+  hp[3] = h[3] - g.W * h[0];
+  hp[4] = h[4] - g.V * hp[2] - g.W * hp[3] - g.q2 * h[0];
+  micro_slope_primed(g, hp, a);
 }
 
-// cubic per weight: u * Px + Py + Pz  (the a_x u + a_y v + a_z w combination of Eq. 5)
-struct UCubic { double d[4][4]; };
+// out (laboratory basis) += B M (primed moments M)
+__device__ __forceinline__ void lab_acc(const Maxw& g, const double* M, double* out) {
+  out[0] += M[0];
+  out[1] += M[1];
+  out[2] = fma(g.V, M[0], out[2] + M[2]);
+  out[3] = fma(g.W, M[0], out[3] + M[3]);
+  out[4] = fma(g.q2, M[0], fma(g.W, M[3], fma(g.V, M[2], out[4] + M[4])));
+}
 
-__device__ __forceinline__ void make_cubic(UCubic& D, const UPoly& px, const UPoly& py, const UPoly& pz) {
-#pragma unroll
-  for (int f = 0; f < 4; f++) {
-    D.d[f][0] = py.c[f][0] + pz.c[f][0];
-    D.d[f][1] = px.c[f][0] + (py.c[f][1] + pz.c[f][1]);
-    D.d[f][2] = px.c[f][1] + (py.c[f][2] + pz.c[f][2]);
-    D.d[f][3] = px.c[f][2];
-  }
+// polynomial in u left by a primed slope after the (c_v, c_w, xi) integrals
+struct SlopePoly { double p[3]; double cv, cw, e4; };      // weight 1: p0 + p1 u + p2 u^2; weights c_v, c_w: constants; e4 = a_4/(2 lam)
+
+__device__ __forceinline__ void make_slope_poly(SlopePoly& P, const Maxw& g, const double* a) {
+  P.p[0] = fma(0.5 * a[4], g.t1, a[0]); P.p[1] = a[1]; P.p[2] = 0.5 * a[4];
+  P.cv = a[2] * g.hil; P.cw = a[3] * g.hil; P.e4 = a[4] * g.hil;
 }
 
 template <int N>
@@ -144,57 +121,74 @@ __device__ __forceinline__ double pdot(const double* c, const double* mu) {
   return s;
 }
 
-// init + sum_k c[k] mu[k] as one FMA chain
-template <int N>
-__device__ __forceinline__ double pdot_acc(const double* c, const double* mu, double init) {
+// primed moments M[alpha] = <(a.psi) u^I psi'_alpha> with the u-moments m (full or half, possibly pre-scaled by rho)
+template <int I>
+__device__ __forceinline__ void apply_slope(const Maxw& g, const SlopePoly& P, const double* m, double* M) {
+  const double d0 = pdot<3>(P.p, m + I), d1 = pdot<3>(P.p, m + I + 1), d2 = pdot<3>(P.p, m + I + 2);
+  M[0] = d0; M[1] = d1; M[2] = P.cv * m[I]; M[3] = P.cw * m[I];
+  M[4] = 0.5 * fma(g.t1, fma(P.e4, m[I], d0), d2);
+}
+
+// shift 0 (conserved moments, MQ) and shift 1 (flux moments, MF) together: the dots d1, d2 are shared
+__device__ __forceinline__ void apply_slope_QF(const Maxw& g, const SlopePoly& P, const double* m, double* MQ, double* MF) {
+  const double d0 = pdot<3>(P.p, m), d1 = pdot<3>(P.p, m + 1), d2 = pdot<3>(P.p, m + 2), d3 = pdot<3>(P.p, m + 3);
+  MQ[0] = d0; MQ[1] = d1; MQ[2] = P.cv * m[0]; MQ[3] = P.cw * m[0];
+  MQ[4] = 0.5 * fma(g.t1, fma(P.e4, m[0], d0), d2);
+  MF[0] = d1; MF[1] = d2; MF[2] = P.cv * m[1]; MF[3] = P.cw * m[1];
+  MF[4] = 0.5 * fma(g.t1, fma(P.e4, m[1], d1), d3);
+}
+
+// The spatial-divergence combination (a_x.psi) u + (a_y.psi) v + (a_z.psi) w of Eq. 5 after the (c_v, c_w, xi) integrals:
+// with v = V + c_v, w = W + c_w and b = V a_y + W a_z it is u (a_x.psi) + (b.psi) + c_v (a_y.psi) + c_w (a_z.psi), which
+// leaves a cubic e(u) for weight 1, quadratics dv(u), dw(u) for weights c_v, c_w and, for weight T,
+// t1 e(u) + (g1 u + g0)/(2 lam).
+struct DivPoly { double e[4], dv[3], dw[3], g0, g1; };
+
+__device__ __forceinline__ void make_div_poly(DivPoly& D, const Maxw& g, const double* ax, const double* ay, const double* az) {
+  const double h = g.hil;
+  double b[5];
 #pragma unroll
-  for (int k = 0; k < N; k++) init = fma(c[k], mu[k], init);
-  return init;
+  for (int k = 0; k < 5; k++) b[k] = fma(g.V, ay[k], g.W * az[k]);
+  const double tr = ay[2] + az[3];
+  const double hb4 = 0.5 * b[4], hx4 = 0.5 * ax[4];
+  D.e[0] = fma(h, tr, fma(hb4, g.t1, b[0]));
+  D.e[1] = fma(hx4, g.t1, ax[0]) + b[1];
+  D.e[2] = ax[1] + hb4;
+  D.e[3] = hx4;
+  const double t1p = fma(2.0, h, g.t1);                     // <c_v^2 T>/<c_v^2> = (K+4)/(2 lam)
+  const double hy4 = 0.5 * ay[4], hz4 = 0.5 * az[4];
+  D.dv[0] = h * (fma(hy4, t1p, ay[0]) + b[2]); D.dv[1] = h * (ax[2] + ay[1]); D.dv[2] = h * hy4;
+  D.dw[0] = h * (fma(hz4, t1p, az[0]) + b[3]); D.dw[1] = h * (ax[3] + az[1]); D.dw[2] = h * hz4;
+  D.g1 = h * (g.t1 * ax[4]);
+  D.g0 = h * fma(g.t1, b[4], 2.0 * (h * tr));
 }
 
-// out[alpha] (+)= < poly u^I psi_alpha > with u-moments mu (full or half, possibly pre-scaled by rho); N = 3 or 4 coefficients.
-// Accumulating variants continue the FMA chain from the accumulator (no separate add).
-template <int N, int I, bool ACC>
-__device__ __forceinline__ void apply_poly(const double (*c)[N], const double* mu, double* out) {
-  const double r4 = pdot_acc<N>(c[3], mu + I, pdot<N>(c[0], mu + I + 2));      // <u^2 .> + <T2 .>
-  if (ACC) {
-    out[0] = pdot_acc<N>(c[0], mu + I, out[0]); out[1] = pdot_acc<N>(c[0], mu + I + 1, out[1]);
-    out[2] = pdot_acc<N>(c[1], mu + I, out[2]); out[3] = pdot_acc<N>(c[2], mu + I, out[3]);
-    out[4] = fma(0.5, r4, out[4]);
-  } else {
-    out[0] = pdot<N>(c[0], mu + I); out[1] = pdot<N>(c[0], mu + I + 1); out[2] = pdot<N>(c[1], mu + I); out[3] = pdot<N>(c[2], mu + I);
-    out[4] = 0.5 * r4;
-  }
+template <int I>
+__device__ __forceinline__ void apply_div(const Maxw& g, const DivPoly& D, const double* m, double* M) {
+  const double e0 = pdot<4>(D.e, m + I), e1 = pdot<4>(D.e, m + I + 1), e2 = pdot<4>(D.e, m + I + 2);
+  M[0] = e0; M[1] = e1; M[2] = pdot<3>(D.dv, m + I); M[3] = pdot<3>(D.dw, m + I);
+  M[4] = 0.5 * fma(g.t1, e0, fma(D.g1, m[I + 1], fma(D.g0, m[I], e2)));
 }
 
-// moments of shift 0 (conserved, outQ) and shift 1 (flux, outF) together: the phi = 1 moments are shared
-template <int N, bool ACC>
-__device__ __forceinline__ void apply_poly_QF(const double (*c)[N], const double* mu, double* outQ, double* outF) {
-  const double e1 = pdot<N>(c[0], mu + 1), e2 = pdot<N>(c[0], mu + 2);
-  const double q4 = pdot_acc<N>(c[3], mu, e2);                                   // <u^2 .> + <T2 .>, shift 0
-  const double f4 = pdot_acc<N>(c[3], mu + 1, pdot<N>(c[0], mu + 3));            // shift 1
-  if (ACC) {
-    outQ[0] = pdot_acc<N>(c[0], mu, outQ[0]); outQ[1] += e1;
-    outQ[2] = pdot_acc<N>(c[1], mu, outQ[2]); outQ[3] = pdot_acc<N>(c[2], mu, outQ[3]); outQ[4] = fma(0.5, q4, outQ[4]);
-    outF[0] += e1; outF[1] += e2;
-    outF[2] = pdot_acc<N>(c[1], mu + 1, outF[2]); outF[3] = pdot_acc<N>(c[2], mu + 1, outF[3]); outF[4] = fma(0.5, f4, outF[4]);
-  } else {
-    outQ[0] = pdot<N>(c[0], mu); outQ[1] = e1; outQ[2] = pdot<N>(c[1], mu); outQ[3] = pdot<N>(c[2], mu); outQ[4] = 0.5 * q4;
-    outF[0] = e1; outF[1] = e2; outF[2] = pdot<N>(c[1], mu + 1); outF[3] = pdot<N>(c[2], mu + 1); outF[4] = 0.5 * f4;
-  }
+__device__ __forceinline__ void apply_div_QF(const Maxw& g, const DivPoly& D, const double* m, double* MQ, double* MF) {
+  const double e0 = pdot<4>(D.e, m), e1 = pdot<4>(D.e, m + 1), e2 = pdot<4>(D.e, m + 2), e3 = pdot<4>(D.e, m + 3);
+  MQ[0] = e0; MQ[1] = e1; MQ[2] = pdot<3>(D.dv, m); MQ[3] = pdot<3>(D.dw, m);
+  MQ[4] = 0.5 * fma(g.t1, e0, fma(D.g1, m[1], fma(D.g0, m[0], e2)));
+  MF[0] = e1; MF[1] = e2; MF[2] = pdot<3>(D.dv, m + 1); MF[3] = pdot<3>(D.dw, m + 1);
+  MF[4] = 0.5 * fma(g.t1, e1, fma(D.g1, m[2], fma(D.g0, m[1], e3)));
 }
 
-// out[alpha] += <u^I psi_alpha> of the plain Maxwellian with (scaled) u-moments mu
+// out[alpha] (laboratory basis) += <u^I psi_alpha> of the plain Maxwellian with (scaled) u-moments mu
 template <int I>
 __device__ __forceinline__ void add_plain(const Maxw& g, const double* mu, double* out) {
   out[0] += mu[I];
   out[1] += mu[I + 1];
-  out[2] += g.V * mu[I];
-  out[3] += g.W * mu[I];
-  out[4] += 0.5 * (mu[I + 2] + g.P2[0][0] * mu[I]);
+  out[2] = fma(g.V, mu[I], out[2]);
+  out[3] = fma(g.W, mu[I], out[3]);
+  out[4] = fma(fma(0.5, g.t1, g.q2), mu[I], fma(0.5, mu[I + 2], out[4]));
 }
 
-struct Groups {        // moments of the groups of Eq. 5 that are shared between both sides (all times rho)
+struct Groups {        // moments of the groups of Eq. 5 that are shared between both sides (all times rho, laboratory basis)
   double W0[5];        // int_{u>0} g_l psi + int_{u<0} g_r psi   (= conserved moments of group 4)
   double dW0[3][5];    // kinetic-weighted slopes of W0 (reading F1)
   double G4F[5];
@@ -202,45 +196,40 @@ struct Groups {        // moments of the groups of Eq. 5 that are shared between
   double G6Q[5], G6F[5];
 };
 
-// one side (SGN = +1: left state, u > 0; SGN = -1: right state, u < 0)
-__device__ __forceinline__ void gks_side(Maxw& g, double mh0, double mh1, const GasConst& gc, const double (*S)[5], Groups& G,
-                                         double* dQs) {
-  maxw_tables(g, gc);
+// one side (left state with the u > 0 half moments, right state with the u < 0 ones)
+__device__ __forceinline__ void gks_side(const Maxw& g, double mh0, double mh1, const double (*S)[5], Groups& G, double* dQs) {
   double mu[6], mh[7];
   mu[0] = 1.0; mu[1] = g.U; mom_recur<6>(mu, g.U, g.hil);
   mh[0] = mh0; mh[1] = mh1;                      // half-space moments, pre-scaled by rho
   mom_recur<7>(mh, g.U, g.hil);
   add_plain<0>(g, mh, G.W0);
   add_plain<1>(g, mh, G.G4F);
-  // micro slopes of the one-sided Maxwellian; divergence cubic
-  double a[5], h[5];
-  UCubic D;
-  {
-    UPoly px, py, pz;
+  // micro slopes of the one-sided Maxwellian (primed basis); their half-space moments feed the slopes of W0
+  double a[3][5], h[5], M[5], MF[5];
 #pragma unroll
-    for (int v = 0; v < 5; v++) h[v] = S[0][v] * g.irho;
-    micro_slope(g, h, a); make_upoly<0, 0>(px, g, a);
-    apply_poly<3, 0, true>(px.c, mh, G.dW0[0]);
+  for (int d = 0; d < 3; d++) {
 #pragma unroll
-    for (int v = 0; v < 5; v++) h[v] = S[1][v] * g.irho;
-    micro_slope(g, h, a); make_upoly<0, 0>(py, g, a);
-    apply_poly<3, 0, true>(py.c, mh, G.dW0[1]);
-    make_upoly<1, 0>(py, g, a);
-#pragma unroll
-    for (int v = 0; v < 5; v++) h[v] = S[2][v] * g.irho;
-    micro_slope(g, h, a); make_upoly<0, 0>(pz, g, a);
-    apply_poly<3, 0, true>(pz.c, mh, G.dW0[2]);
-    make_upoly<0, 1>(pz, g, a);
-    make_cubic(D, px, py, pz);
+    for (int v = 0; v < 5; v++) h[v] = S[d][v] * g.irho;
+    micro_slope_lab(g, h, a[d]);
+    SlopePoly P; make_slope_poly(P, g, a[d]);
+    apply_slope<0>(g, P, mh, M);
+    lab_acc(g, M, G.dW0[d]);
   }
-  // time slope from the compatibility condition <a_x u + a_y v + a_z w + A> = 0 (full velocity space)
-  apply_poly<4, 0, false>(D.d, mu, h);
+  DivPoly D; make_div_poly(D, g, a[0], a[1], a[2]);
+  // time slope from the compatibility condition <a_x u + a_y v + a_z w + A> = 0 (full velocity space): the primed
+  // moments go straight into the primed solve
+  apply_div<0>(g, D, mu, M);
 #pragma unroll
-  for (int v = 0; v < 5; v++) { h[v] = -h[v]; dQs[v] = g.rho * h[v]; }     // d/dt of the one-sided Maxwellian's moments
-  apply_poly_QF<4, true>(D.d, mh, G.G5Q, G.G5F);
-  micro_slope(g, h, a);
-  UPoly pa; make_upoly<0, 0>(pa, g, a);
-  apply_poly_QF<3, true>(pa.c, mh, G.G6Q, G.G6F);
+  for (int v = 0; v < 5; v++) { M[v] = -M[v]; dQs[v] = 0.0; }
+  lab_acc(g, M, dQs);
+#pragma unroll
+  for (int v = 0; v < 5; v++) dQs[v] *= g.rho;                                // d/dt of the one-sided Maxwellian's moments
+  double A[5]; micro_slope_primed(g, M, A);
+  apply_div_QF(g, D, mh, M, MF);
+  lab_acc(g, M, G.G5Q); lab_acc(g, MF, G.G5F);
+  SlopePoly PA; make_slope_poly(PA, g, A);
+  apply_slope_QF(g, PA, mh, M, MF);
+  lab_acc(g, M, G.G6Q); lab_acc(g, MF, G.G6F);
 }
 
 // time-integrated coefficients of the six groups of Eq. 5 over [0,T]
@@ -267,7 +256,7 @@ __device__ __forceinline__ void gks_flux_local(const GasConst& gc, double dt, do
     G.dW0[0][v] = 0; G.dW0[1][v] = 0; G.dW0[2][v] = 0;
   }
   // scalars and half-space moments of both sides first: the two erfc/exp/sqrt/reciprocal chains are independent and
-  // overlap in the FP64 pipe; the tables and slopes of each side follow
+  // overlap in the FP64 pipe; the slopes of each side follow
   double pl, pr;
   {
     Maxw gl, gr;
@@ -275,35 +264,34 @@ __device__ __forceinline__ void gks_flux_local(const GasConst& gc, double dt, do
     maxw_scalars(gl, WL, gc); maxw_scalars(gr, WR, gc);
     half_moments(gl, 1.0, hl0, hl1); half_moments(gr, -1.0, hr0, hr1);
     pl = gl.rho * gl.hil; pr = gr.rho * gr.hil;
-    gks_side(gl, hl0, hl1, gc, SL, G, DL);     // DL, DR hold the one-sided time derivatives for now
-    gks_side(gr, hr0, hr1, gc, SR, G, DR);
+    gks_side(gl, hl0, hl1, SL, G, DL);     // DL, DR hold the one-sided time derivatives for now
+    gks_side(gr, hr0, hr1, SR, G, DR);
   }
   // equilibrium state g0 and its slopes
-  Maxw g0; maxw_scalars(g0, G.W0, gc); maxw_tables(g0, gc);
+  Maxw g0; maxw_scalars(g0, G.W0, gc);
   double mu[7];
   mu[0] = g0.rho; mu[1] = g0.rho * g0.U; mom_recur<7>(mu, g0.U, g0.hil);     // full moments times rho0
-  double G1F[5] = { 0, 0, 0, 0, 0 }, G2Q[5], G2F[5], G3F[5];
+  double G1F[5] = { 0, 0, 0, 0, 0 }, G2Q[5] = { 0, 0, 0, 0, 0 }, G2F[5] = { 0, 0, 0, 0, 0 }, G3F[5] = { 0, 0, 0, 0, 0 };
   add_plain<1>(g0, mu, G1F);
-  double a[5], h[5];
   {
-    UCubic D; UPoly px, py, pz;
+    double a[3][5], h[5], MQ[5], MF[5];
 #pragma unroll
-    for (int v = 0; v < 5; v++) h[v] = G.dW0[0][v] * g0.irho;
-    micro_slope(g0, h, a); make_upoly<0, 0>(px, g0, a);
+    for (int d = 0; d < 3; d++) {
 #pragma unroll
-    for (int v = 0; v < 5; v++) h[v] = G.dW0[1][v] * g0.irho;
-    micro_slope(g0, h, a); make_upoly<1, 0>(py, g0, a);
+      for (int v = 0; v < 5; v++) h[v] = G.dW0[d][v] * g0.irho;
+      micro_slope_lab(g0, h, a[d]);
+    }
+    DivPoly D; make_div_poly(D, g0, a[0], a[1], a[2]);
+    apply_div_QF(g0, D, mu, MQ, MF);
+    lab_acc(g0, MQ, G2Q); lab_acc(g0, MF, G2F);
+    // Abar from <abar.u + Abar> = 0: its primed conserved moments are -MQ
 #pragma unroll
-    for (int v = 0; v < 5; v++) h[v] = G.dW0[2][v] * g0.irho;
-    micro_slope(g0, h, a); make_upoly<0, 1>(pz, g0, a);
-    make_cubic(D, px, py, pz);
-    apply_poly_QF<4, false>(D.d, mu, G2Q, G2F);
+    for (int v = 0; v < 5; v++) h[v] = -MQ[v] * g0.irho;
+    double A[5]; micro_slope_primed(g0, h, A);
+    SlopePoly PA; make_slope_poly(PA, g0, A);
+    apply_slope<1>(g0, PA, mu, MF);
+    lab_acc(g0, MF, G3F);
   }
-  // Abar from <abar.u + Abar> = 0; its conserved moments are -G2Q
-#pragma unroll
-  for (int v = 0; v < 5; v++) h[v] = -G2Q[v] * g0.irho;
-  micro_slope(g0, h, a);
-  { UPoly pa; make_upoly<0, 0>(pa, g0, a); apply_poly<3, 1, false>(pa.c, mu, G3F); }
   // collision time
   double tau_phys = 0.0;
   if (gc.mu_ref > 0.0) {
