@@ -358,7 +358,7 @@ extern "C" int cgks_debug_stage(cgks_ctx* c, double dt, double* d_pv, double* d_
   if (m.cart) recon_kernel<true><<<grid, TPB, 0, c->stream>>>(m, sl, Win, c->pv, c->chi, rp, 0, nt, c->d_flags + 3);
   else recon_kernel<false><<<grid, TPB, 0, c->stream>>>(m, sl, Win, c->pv, c->chi, rp, 0, nt, c->d_flags + 3);
   c->launches++;
-  if (d_pv) CK(cudaMemcpyAsync(d_pv, c->pv, (size_t)NPV * m.n * 8, cudaMemcpyDeviceToDevice, c->stream));
+  if (d_pv) { pv_unpack_kernel<<<dim3((unsigned)((nt + TPB - 1) / TPB), 24 * NVAR), TPB, 0, c->stream>>>(sl, m.n, c->pv, d_pv); c->launches++; }
   if (d_fx) {
     if (m.cart) launch_flux<true>(c, sl, Win, dt, 0, m.nk, 1); else launch_flux<false>(c, sl, Win, dt, 0, m.nk, 1);
     CK(cudaMemcpyAsync(d_fx, c->fx, (size_t)NFX * m.n * 8, cudaMemcpyDeviceToDevice, c->stream));

@@ -8,7 +8,7 @@ namespace cgks {
 // ---- HBM layout (all fp64, structure-of-arrays, i fastest) ---------------------------------------------------------
 // state buffer        [80][N]      planes: Q v (0..4) | G 5+3v+r (5..19) | D 20+12v+s (20..79)
 // metrics (general)   [37][N]      J0 3r+a (0..8) | J0^-1 9+3a+r... see MET_* | vol | +face vector areas | +face tangents
-// pv (slab)           [480][slots*plane]   plane (4m+q)*20 + c : c = v (value) | 5+3v+r (physical gradient)
+// pv (slab)           [24*5][slots*plane][4]   record (point p = 4m+q, variable v, cell slot) = { value, physical gradient (3) }
 // fx (slab)           [360][slots*plane]   plane (4ax+q)*30 + c : Fn 0..4 | Ft 5..9 | VL 10..14 | DL 15..19 | VR 20..24 | DR 25..29
 enum { NVAR = 5, NSTATE = 80, NPV = 480, NFX = 360, NMET = 37 };
 enum { MET_J0 = 0, MET_J0INV = 9, MET_VOL = 18, MET_AREA = 19, MET_TAN = 28 };

@@ -14,6 +14,13 @@ struct ReconPrm { int nonlinear; double C, eps, inv_tanhC, gamma; };
 // pv and fx are written once and read once by the next kernel, far beyond the L2 capacity: streaming (evict-first) stores.
 // (Streaming LOADS of fx in the update kernel were 24 % slower: the face values shared with the neighbours do hit in L2.)
 #define ST_STREAM(p, v) __stcs((p), (v))
+// pv record of one (Gauss point p, variable v, cell slot): { value, d/dx, d/dy, d/dz } = 32 contiguous bytes, written with ONE
+// 256-bit streaming store and read by the flux kernel with two 16-byte cp.async (a quarter / half of the memory instructions of
+// a plane-per-component layout, and 1 KB contiguous per warp).  Index of the record's first double:
+__device__ __forceinline__ long pv_index(const Slab& sl, int p, int v, long off) { return ((long)(p * NVAR + v) * sl.stride_pv + off) * 4; }
+__device__ __forceinline__ void st_stream4(double* dst, double a, double b, double c, double d) {
+  asm volatile("st.global.cs.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(__cvta_generic_to_global(dst)), "d"(a), "d"(b), "d"(c), "d"(d) : "memory");
+}
 #ifndef FLUX_MINB
 #define FLUX_MINB 2
 #endif
@@ -165,22 +172,30 @@ __global__ void __launch_bounds__(128, 3) recon_kernel(Mesh m, Slab sl, const do
 #pragma unroll
     for (int l = 0; l < 8; l++) {
       const int p = 8 * ax + l;            // = 4 * (2 ax + sgn) + 2a + b
-      double* dst = pv + (long)(p * 20) * sl.stride_pv + off;
-      ST_STREAM(dst + (long)v * sl.stride_pv, q0 + o[4 * l]);
       double g[3];
       if (CART) { g[0] = o[4 * l + 1] * ih[0]; g[1] = o[4 * l + 2] * ih[1]; g[2] = o[4 * l + 3] * ih[2]; }
       else {
 #pragma unroll
         for (int r = 0; r < 3; r++) g[r] = Ji[r] * o[4 * l + 1] + Ji[3 + r] * o[4 * l + 2] + Ji[6 + r] * o[4 * l + 3];
       }
-#pragma unroll
-      for (int r = 0; r < 3; r++) ST_STREAM(dst + (long)(5 + 3 * v + r) * sl.stride_pv, g[r]);
+      st_stream4(pv + pv_index(sl, p, v, off), q0 + o[4 * l], g[0], g[1], g[2]);
     }
   };
   if (VOLUME) { double o[32]; recon_eval_volume(a, o); store_axis(0, o); return; }
   { double o[32]; eval_axis<0>(a, o); store_axis(0, o); }
   { double o[32]; eval_axis<1>(a, o); store_axis(1, o); }
   { double o[32]; eval_axis<2>(a, o); store_axis(2, o); }
+}
+
+// test tap: pv records -> planes [480][n] in the documented order (plane (4m+q)*20 + c: c = v value, 5+3v+r gradient)
+__global__ void pv_unpack_kernel(Slab sl, long n, const double* __restrict__ pv, double* __restrict__ out) {
+  const long c = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= n) return;
+  const int pvv = blockIdx.y, p = pvv / NVAR, v = pvv - p * NVAR;
+  const double* src = pv + pv_index(sl, p, v, c);
+  out[(long)(p * 20 + v) * n + c] = src[0];
+#pragma unroll
+  for (int r = 0; r < 3; r++) out[(long)(p * 20 + 5 + 3 * v + r) * n + c] = src[1 + r];
 }
 
 // ------------------------------------------------------------------------------------------------ diagnostics
@@ -201,14 +216,13 @@ __global__ void __launch_bounds__(128) diag_kernel(Mesh m, Slab sl, const double
     vol = CART ? m.h[0] * m.h[1] * m.h[2] : m.met[MET_VOL * m.n + x.c];
 #pragma unroll 1
     for (int p = 0; p < 8; p++) {
-      const double* src = pv + (long)(p * 20) * sl.stride_pv + off;
       double w[5], g[4][3];
 #pragma unroll
-      for (int c = 0; c < 5; c++) w[c] = src[(long)c * sl.stride_pv];
-#pragma unroll
-      for (int c = 0; c < 4; c++)
-#pragma unroll
-        for (int r = 0; r < 3; r++) g[c][r] = src[(long)(5 + 3 * c + r) * sl.stride_pv];
+      for (int c = 0; c < 5; c++) {
+        const double* src = pv + pv_index(sl, p, c, off);
+        w[c] = src[0];
+        if (c < 4) { g[c][0] = src[1]; g[c][1] = src[2]; g[c][2] = src[3]; }
+      }
       double pe = w[4] - 0.5 * (w[1] * w[1] + w[2] * w[2] + w[3] * w[3]) / w[0];
       if (!admissible(w)) {                    // positivity fallback (reading R9): cell average, zero gradient
 #pragma unroll
@@ -269,10 +283,10 @@ __global__ void __launch_bounds__(256) diag_reduce_kernel(const double* __restri
 // shared-memory tile (refilled for the next tile as soon as it has been read into registers), one tile ahead, so the DRAM latency of the loads is hidden
 // behind the ~2000 FP64 instructions of the previous point (no block-level synchronisation is needed: a thread only
 // reads what it copied).
-__device__ __forceinline__ void cp_async8(double* smem_dst, const double* gsrc) {
+__device__ __forceinline__ void cp_async16(double* smem_dst, const double* gsrc) {
   const unsigned sa = (unsigned)__cvta_generic_to_shared(smem_dst);
   const size_t ga = __cvta_generic_to_global(gsrc);          // the instruction takes a .global address, not a generic one
-  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(sa), "l"(ga) : "memory");
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 16;\n" ::"r"(sa), "l"(ga) : "memory");
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
 template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
@@ -299,7 +313,7 @@ __device__ __forceinline__ bool flux_point(const Mesh& m, const Slab& sl, long t
 template <bool CART, int AXIS, bool STAGE2>
 __global__ void __launch_bounds__(FLUX_TPB, FLUX_MINB) flux_kernel(Mesh m, Slab sl, const double* __restrict__ W, const double* __restrict__ pv,
                                                    double* __restrict__ fx, GasConst gc, double dt, double idt, int kA, long ncells) {
-  extern __shared__ double smf[];                     // [40][FLUX_TPB]
+  extern __shared__ __align__(16) double smf[];       // [20 chunks][FLUX_TPB][2]
   const long tiles_per_q = (ncells + FLUX_TPB - 1) / FLUX_TPB;
   const long ntiles = 4 * tiles_per_q;
   // returns whether this thread has a point in `tile`; its q and left offset are carried to the compute phase
@@ -307,17 +321,14 @@ __global__ void __launch_bounds__(FLUX_TPB, FLUX_MINB) flux_kernel(Mesh m, Slab 
     FluxPoint f;
     const bool act = tile < ntiles && flux_point<AXIS>(m, sl, tile, tiles_per_q, ncells, kA, f);
     if (act) {
-      const double* pL = pv + f.offL;
-      const double* pR = pv + f.offR;
-      // NOTE: keep the plane index inside each copy's address expression.  With the base pointers written as
-      // pv + plane * stride + off and advanced by c * stride, nvcc 12.9 / sm_100a produced the RIGHT face's plane for
-      // the left copies of AXIS = 2 (caught by the parity tests; the echo of the staged values showed it).
-      const long planeL = (long)((4 * (2 * AXIS) + f.q) * 20), planeR = (long)((4 * (2 * AXIS + 1) + f.q) * 20);
-      double* dstL = smf + threadIdx.x;
+      // chunk (side, variable, half) = 16 bytes: { value, d/dx } or { d/dy, d/dz }; tile layout [20 chunks][FLUX_TPB][2]
+      const double* pL = pv + pv_index(sl, 4 * (2 * AXIS) + f.q, 0, f.offL);
+      const double* pR = pv + pv_index(sl, 4 * (2 * AXIS + 1) + f.q, 0, f.offR);
+      double* dst = smf + 2 * threadIdx.x;
 #pragma unroll
-      for (int c = 0; c < 20; c++) cp_async8(dstL + c * FLUX_TPB, pL + (planeL + c) * sl.stride_pv);
+      for (int c = 0; c < 10; c++) cp_async16(dst + c * (2 * FLUX_TPB), pL + (long)(c >> 1) * (4 * sl.stride_pv) + 2 * (c & 1));
 #pragma unroll
-      for (int c = 0; c < 20; c++) cp_async8(dstL + (20 + c) * FLUX_TPB, pR + (planeR + c) * sl.stride_pv);
+      for (int c = 0; c < 10; c++) cp_async16(dst + (10 + c) * (2 * FLUX_TPB), pR + (long)(c >> 1) * (4 * sl.stride_pv) + 2 * (c & 1));
       q_out = f.q; offL_out = f.offL; c_out = f.x.c;
     }
     cp_async_commit();
@@ -329,12 +340,15 @@ __global__ void __launch_bounds__(FLUX_TPB, FLUX_MINB) flux_kernel(Mesh m, Slab 
 #pragma unroll 1
   for (long tile = blockIdx.x; tile < ntiles; tile += gridDim.x, q = qn, offL = offLn, cL = cLn, active = activen) {
   cp_async_wait<0>();
-  const double* sL = smf + threadIdx.x;
+  const double2* sL = reinterpret_cast<const double2*>(smf) + threadIdx.x;
   double WLg[5], WRg[5], gL[15], gR[15];
 #pragma unroll
-  for (int c = 0; c < 5; c++) { WLg[c] = sL[c * FLUX_TPB]; WRg[c] = sL[(20 + c) * FLUX_TPB]; }
-#pragma unroll
-  for (int c = 0; c < 15; c++) { gL[c] = sL[(5 + c) * FLUX_TPB]; gR[c] = sL[(25 + c) * FLUX_TPB]; }
+  for (int v = 0; v < 5; v++) {
+    const double2 l0 = sL[(2 * v) * FLUX_TPB], l1 = sL[(2 * v + 1) * FLUX_TPB];
+    const double2 r0 = sL[(10 + 2 * v) * FLUX_TPB], r1 = sL[(11 + 2 * v) * FLUX_TPB];
+    WLg[v] = l0.x; gL[3 * v] = l0.y; gL[3 * v + 1] = l1.x; gL[3 * v + 2] = l1.y;
+    WRg[v] = r0.x; gR[3 * v] = r0.y; gR[3 * v + 1] = r1.x; gR[3 * v + 2] = r1.y;
+  }
   activen = issue(tile + gridDim.x, qn, offLn, cLn);      // next tile's inputs stream in while this point is computed
   if (!active) continue;
   // positivity (reading R9, point-wise): a non-physical reconstructed state falls back to the cell average
