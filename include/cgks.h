@@ -80,6 +80,31 @@ int cgks_compute_dt(cgks_ctx*, double cfl, double* dt_host);
 /* One two-stage fourth-order step of size dt.  Asynchronous. */
 int cgks_step(cgks_ctx*, double dt);
 
+/* One stage of the step (1: state n -> stage state; 2: stage state -> state n+1); cgks_step(dt) is
+   cgks_stage(1, dt) followed by cgks_stage(2, dt).  Stages must alternate 1, 2.  Asynchronous. */
+int cgks_stage(cgks_ctx*, int stage, double dt);
+
+/* ---- Sub-domains of a slab decomposition along k (the paper's own parallelisation: "domain decomposed
+   into slabs along one dimension", one rank per GPU) -------------------------------------
+   A sub-domain context holds nk_owned k-planes of the global periodic mesh starting at global plane k0, plus TWO halo
+   planes on each side (a cell's update needs the state of cells within index distance 2 per stage): its arrays have
+   nk_owned + 4 planes, local plane 2 being global plane k0.  d_nodes is the node array of the WHOLE mesh
+   [3][nk_global+1][nj+1][ni+1] (read during the call only), so that every cell has bit-identical metrics whichever
+   context holds it.  Before EACH stage the halo planes of the stage's input state must be current:
+       cgks_pack_halo(side) on the neighbour  ->  transport (NCCL / peer copy; the caller's)  ->  cgks_unpack_halo(side),
+   side 0 = low k, 1 = high k; pack copies the two outermost OWNED planes of that side, unpack fills the two HALO planes
+   of that side, all 80 fields, buffer layout [80][2][nj][ni] (cgks_halo_bytes).  Between cgks_stage(1) and cgks_stage(2)
+   the calls act on the stage state, otherwise on the current state.  cgks_set_state / cgks_get_state take arrays of
+   nk_owned + 4 planes (halo planes of Q should hold the neighbours' values so that the bootstrap of reading S2 is right
+   on the owned planes; halo planes returned by cgks_get_state are not current).  cgks_compute_dt reduces over the owned
+   planes only: the caller takes the minimum over sub-domains (one scalar all-reduce per step).  cgks_step,
+   cgks_run_host, cgks_diagnostics and the debug taps need a whole-mesh context. */
+int cgks_create_slab(cgks_ctx** out, int ni, int nj, int nk_global, int k0, int nk_owned, const double* d_nodes,
+                     const cgks_params* params, void* d_workspace, size_t workspace_bytes, void* cuda_stream);
+int cgks_halo_bytes(const cgks_ctx*, size_t* bytes);
+int cgks_pack_halo(cgks_ctx*, int side, double* d_buf);
+int cgks_unpack_halo(cgks_ctx*, int side, const double* d_buf);
+
 /* Diagnostics of the current state: volume-averaged kinetic energy E_k = int rho |U|^2/2 dV / |Omega| and
    enstrophy int mu |curl U|^2 dV / |Omega| (rho_0 = 1), by the 2x2x2 Gauss rule on every cell with values and velocity
    derivatives from the compact reconstruction (the scheme's own polynomial, Eq. 16; reading X1); mu is the

@@ -46,6 +46,11 @@ def lib():
         L.cgks_get_state.argtypes = [_vp, _vp, _vp, _vp]
         L.cgks_compute_dt.argtypes = [_vp, C.c_double, C.POINTER(C.c_double)]
         L.cgks_step.argtypes = [_vp, C.c_double]
+        L.cgks_stage.argtypes = [_vp, C.c_int, C.c_double]
+        L.cgks_create_slab.argtypes = [C.POINTER(_vp), C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, _vp, C.POINTER(cgks_params), _vp, C.c_size_t, _vp]
+        L.cgks_halo_bytes.argtypes = [_vp, C.POINTER(C.c_size_t)]
+        L.cgks_pack_halo.argtypes = [_vp, C.c_int, _vp]
+        L.cgks_unpack_halo.argtypes = [_vp, C.c_int, _vp]
         L.cgks_status.argtypes = [_vp]
         L.cgks_diagnostics.argtypes = [_vp, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.cgks_run_host.argtypes = [_vp, _vp, _vp, _vp, C.c_double, C.c_int, _vp, _vp, _vp]
@@ -118,22 +123,30 @@ class Solver:
 
     nodes (3, nk+1, nj+1, ni+1); Q (5, nk, nj, ni); G (5, 3, nk, nj, ni); D (5, 12, nk, nj, ni)."""
 
-    def __init__(self, nodes, params, device="cuda:0", budget_bytes=0, workspace_nbytes=None):
+    def __init__(self, nodes, params, device="cuda:0", budget_bytes=0, workspace_nbytes=None, slab=None):
+        """slab = (k0, nk_owned): a sub-domain context (cgks_create_slab) of the global mesh given by `nodes`; its arrays
+        have nk_owned + 4 planes (two halo planes on each side)."""
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2508_08965_b200 needs a CUDA device (no CPU fallback)")
         self.device = torch.device(device)
         self._h = _vp(None)
         L = lib()
         nodes = _dev(nodes, self.device)
-        self.nk, self.nj, self.ni = (int(s) - 1 for s in nodes.shape[1:])
+        self.nk_global, self.nj, self.ni = (int(s) - 1 for s in nodes.shape[1:])
+        self.slab = slab
+        self.nk = self.nk_global if slab is None else int(slab[1]) + 4
         self.n = self.ni * self.nj * self.nk
         self.params = params if isinstance(params, cgks_params) else make_params(**params)
         nbytes = workspace_nbytes or workspace_bytes(self.ni, self.nj, self.nk, budget_bytes)
         with torch.cuda.device(self.device):
             self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
             self.stream = torch.cuda.current_stream(self.device)
-            rc = L.cgks_create(C.byref(self._h), self.ni, self.nj, self.nk, _ptr(nodes), C.byref(self.params),
-                               _vp(self.workspace.data_ptr()), nbytes, _vp(self.stream.cuda_stream))
+            if slab is None:
+                rc = L.cgks_create(C.byref(self._h), self.ni, self.nj, self.nk, _ptr(nodes), C.byref(self.params),
+                                   _vp(self.workspace.data_ptr()), nbytes, _vp(self.stream.cuda_stream))
+            else:
+                rc = L.cgks_create_slab(C.byref(self._h), self.ni, self.nj, self.nk_global, int(slab[0]), int(slab[1]), _ptr(nodes),
+                                        C.byref(self.params), _vp(self.workspace.data_ptr()), nbytes, _vp(self.stream.cuda_stream))
         if rc:
             self._h = _vp(None)
             raise CgksError(rc, "cgks_create: " + L.cgks_last_create_error().decode())
@@ -174,6 +187,21 @@ class Solver:
 
     def step(self, dt):
         self._check(lib().cgks_step(self._h, float(dt)))
+
+    def stage(self, stage, dt):
+        self._check(lib().cgks_stage(self._h, int(stage), float(dt)))
+
+    def halo_buffer(self):
+        """A device buffer for one side's halo planes, [80][2][nj][ni] (cgks_halo_bytes)."""
+        nb = C.c_size_t(0)
+        self._check(lib().cgks_halo_bytes(self._h, C.byref(nb)))
+        return torch.empty(nb.value // 8, dtype=torch.float64, device=self.device)
+
+    def pack_halo(self, side, buf):
+        self._check(lib().cgks_pack_halo(self._h, int(side), _ptr(buf)))
+
+    def unpack_halo(self, side, buf):
+        self._check(lib().cgks_unpack_halo(self._h, int(side), _ptr(buf)))
 
     def diagnostics(self):
         """(E_k, enstrophy) of the current state, divided by |Omega|."""

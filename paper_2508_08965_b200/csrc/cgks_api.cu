@@ -39,6 +39,9 @@ struct cgks_ctx {
   unsigned long long* d_dt = nullptr;   // [1] bit pattern of the reduced dt
   int* d_flags = nullptr;               // [0..2] geometry, [3] non-physical state
   int nsm = 148;                        // multiprocessors of the device
+  int open_k = 0;                       // 1: sub-domain of a slab decomposition along k (2 halo planes on each side)
+  int kofs = 0, nk_global = 0;          // global plane of local plane 0 (may be negative: wraps), planes of the global mesh
+  int phase = 0;                        // sub-domain: 0 = next is stage 1 (input W[cur]), 1 = next is stage 2 (input W[star])
   int S = 0;                            // slab depth in k-planes; S == nk: whole mesh resident
   int slots_pv = 0, slots_fx = 0;
   long launches = 0;
@@ -133,12 +136,14 @@ static cudaError_t set_flux_smem() {
 }
 
 // ---- create / destroy -------------------------------------------------------------------------------------------
-extern "C" int cgks_create(cgks_ctx** out, int ni, int nj, int nk, const double* d_nodes, const cgks_params* params,
-                           void* ws, size_t ws_bytes, void* stream) {
+// nkg = planes of the global mesh (the node array), nk = planes held by this context starting at global plane kofs
+static int create_impl(cgks_ctx** out, int ni, int nj, int nkg, int nk, int kofs, int open_k, const double* d_nodes, const cgks_params* params,
+                       void* ws, size_t ws_bytes, void* stream) {
   if (!out) return CGKS_EINVAL;
   *out = nullptr;
   auto early = [&](int code, const char* msg) { g_create_err = msg; return code; };
-  if (ni < 4 || nj < 4 || nk < 4) return early(CGKS_EINVAL, "ni, nj, nk must be at least 4");
+  if (ni < 4 || nj < 4 || nkg < 4) return early(CGKS_EINVAL, "ni, nj, nk must be at least 4");
+  if (open_k && nk < 6) return early(CGKS_EINVAL, "a sub-domain must own at least 2 planes");
   if (!d_nodes || !params || !ws) return early(CGKS_EINVAL, "null argument");
   if ((double)ni * nj * nk >= 2147483648.0 / 8.0) return early(CGKS_EINVAL, "mesh too large for 32-bit cell indices");      // 32-bit cell and tile indices in the kernels
   if (params->geno_r != 2 || !(params->gamma > 1.0) || !(params->gamma < 5.0 / 3.0 + 1e-12)) return early(CGKS_EINVAL, "unsupported parameters (geno_r must be 2, 1 < gamma <= 5/3)");
@@ -146,6 +151,7 @@ extern "C" int cgks_create(cgks_ctx** out, int ni, int nj, int nk, const double*
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return early(CGKS_ECUDA, "no CUDA device");
   cgks_ctx* c = new cgks_ctx();
   c->prm = *params; c->stream = (cudaStream_t)stream;
+  c->open_k = open_k; c->kofs = kofs; c->nk_global = nkg;
   {
     int dev = 0; cudaGetDevice(&dev);
     if (cudaDeviceGetAttribute(&c->nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || c->nsm <= 0) c->nsm = 148;
@@ -168,7 +174,7 @@ extern "C" int cgks_create(cgks_ctx** out, int ni, int nj, int nk, const double*
     if (cudaMemsetAsync(c->d_flags, 0, 64, c->stream) != cudaSuccess) { bail(CGKS_ECUDA, "cudaMemsetAsync failed"); break; }
     const unsigned gridg = (unsigned)((n + TPB - 1) / TPB);
     // pass 1: validity + uniform-Cartesian detection (no metric storage)
-    geometry_kernel<<<gridg, TPB, 0, c->stream>>>(ni, nj, nk, d_nodes, nullptr, c->d_flags); c->launches++;
+    geometry_kernel<<<gridg, TPB, 0, c->stream>>>(ni, nj, nkg, nk, kofs, d_nodes, nullptr, c->d_flags); c->launches++;
     int flags[4] = { 0, 0, 0, 0 };
     cudaError_t e = cudaMemcpyAsync(flags, c->d_flags, sizeof flags, cudaMemcpyDeviceToHost, c->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
@@ -178,7 +184,7 @@ extern "C" int cgks_create(cgks_ctx** out, int ni, int nj, int nk, const double*
     m.cart = flags[0] ? 0 : 1;
     if (m.cart) {
       // h = period / n from four corner nodes
-      const long ns = (long)(ni + 1) * (nj + 1) * (nk + 1);
+      const long ns = (long)(ni + 1) * (nj + 1) * (nkg + 1);
       auto node = [&](int comp, int i, int j, int k, double* v) {
         return cudaMemcpy(v, d_nodes + comp * ns + ((long)k * (nj + 1) + j) * (ni + 1) + i, 8, cudaMemcpyDeviceToHost);
       };
@@ -186,12 +192,12 @@ extern "C" int cgks_create(cgks_ctx** out, int ni, int nj, int nk, const double*
       for (int r = 0; r < 3; r++) node(r, 0, 0, 0, &o[r]);
       node(0, ni, 0, 0, &a); m.h[0] = (a - o[0]) / ni;
       node(1, 0, nj, 0, &a); m.h[1] = (a - o[1]) / nj;
-      node(2, 0, 0, nk, &a); m.h[2] = (a - o[2]) / nk;
+      node(2, 0, 0, nkg, &a); m.h[2] = (a - o[2]) / nkg;
     } else {
       if (p + align_up((size_t)NMET * n * 8) > end) { bail(CGKS_ENOMEM, "workspace too small for the mesh metrics"); break; }
       c->met = (double*)p; p += align_up((size_t)NMET * n * 8);
       m.met = c->met;
-      geometry_kernel<<<gridg, TPB, 0, c->stream>>>(ni, nj, nk, d_nodes, c->met, c->d_flags); c->launches++;
+      geometry_kernel<<<gridg, TPB, 0, c->stream>>>(ni, nj, nkg, nk, kofs, d_nodes, c->met, c->d_flags); c->launches++;
       e = cudaStreamSynchronize(c->stream);
       if (e != cudaSuccess) { c->err = std::string("geometry pass 2: ") + cudaGetErrorString(e); rc = CGKS_ECUDA; break; }
     }
@@ -217,6 +223,17 @@ extern "C" int cgks_create(cgks_ctx** out, int ni, int nj, int nk, const double*
   return CGKS_OK;
 }
 
+extern "C" int cgks_create(cgks_ctx** out, int ni, int nj, int nk, const double* d_nodes, const cgks_params* params,
+                           void* ws, size_t ws_bytes, void* stream) {
+  return create_impl(out, ni, nj, nk, nk, 0, 0, d_nodes, params, ws, ws_bytes, stream);
+}
+
+extern "C" int cgks_create_slab(cgks_ctx** out, int ni, int nj, int nk_global, int k0, int nk_owned, const double* d_nodes,
+                                const cgks_params* params, void* ws, size_t ws_bytes, void* stream) {
+  if (nk_owned < 2 || nk_owned > nk_global || k0 < 0 || k0 >= nk_global) { g_create_err = "bad slab range"; if (out) *out = nullptr; return CGKS_EINVAL; }
+  return create_impl(out, ni, nj, nk_global, nk_owned + 4, k0 - 2, 1, d_nodes, params, ws, ws_bytes, stream);
+}
+
 extern "C" int cgks_destroy(cgks_ctx* c) {
   if (!c) return CGKS_EINVAL;
   cudaStreamSynchronize(c->stream);
@@ -229,6 +246,7 @@ extern "C" int cgks_destroy(cgks_ctx* c) {
 // ---- state ------------------------------------------------------------------------------------------------------
 extern "C" int cgks_set_state(cgks_ctx* c, const double* Q, const double* G, const double* D) {
   if (!c || !Q) return CGKS_EINVAL;
+  c->phase = 0;
   const Mesh& m = c->mesh;
   dim3 grid((unsigned)((m.n + TPB - 1) / TPB), 5);
   { Timed t(c, KC_OTHER); set_state_kernel<<<grid, TPB, 0, c->stream>>>(m, Q, G, D, c->W[c->cur]); }
@@ -270,7 +288,8 @@ extern "C" int cgks_compute_dt(cgks_ctx* c, double cfl, double* dt_host) {
   CK(cudaMemcpyAsync(c->d_dt, &inf_bits, 8, cudaMemcpyHostToDevice, c->stream));
   CflPrm p{ c->prm.gamma, c->prm.mu_ref, c->prm.visc_omega, c->prm.T_ref, cfl };
   long blocks = (m.n + 255) / 256; if (blocks > (long)c->nsm * 16) blocks = (long)c->nsm * 16;
-  { Timed t(c, KC_CFL); cfl_kernel<<<(unsigned)blocks, 256, 0, c->stream>>>(m, c->W[c->cur], p, c->d_dt, c->d_flags + 3); }
+  const int kA = c->open_k ? 2 : 0, cnt = c->open_k ? m.nk - 4 : m.nk;
+  { Timed t(c, KC_CFL); cfl_kernel<<<(unsigned)blocks, 256, 0, c->stream>>>(m, c->W[c->cur], p, c->d_dt, c->d_flags + 3, kA, cnt); }
   unsigned long long bits = 0; int flag = 0;
   CK(cudaMemcpyAsync(&bits, c->d_dt, 8, cudaMemcpyDeviceToHost, c->stream));
   CK(cudaMemcpyAsync(&flag, c->d_flags + 3, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
@@ -320,11 +339,16 @@ static void run_stage(cgks_ctx* c, int stage, double dt) {
   };
   if (c->S >= m.nk) {                       // whole mesh resident: no recomputation
     sl.kbase = 0;
-    recon(0, m.nk); launch_flux<CART>(c, sl, Win, dt, 0, m.nk, stage); update(0, m.nk);
+    if (c->open_k) {                        // sub-domain: planes 0, 1 and nk-2, nk-1 are halos (filled by cgks_unpack_halo)
+      recon(1, m.nk - 2); launch_flux<CART>(c, sl, Win, dt, 1, m.nk - 3, stage); update(2, m.nk - 4);
+    } else {
+      recon(0, m.nk); launch_flux<CART>(c, sl, Win, dt, 0, m.nk, stage); update(0, m.nk);
+    }
     return;
   }
-  for (int k0 = 0; k0 < m.nk; k0 += c->S) {
-    const int k1 = (k0 + c->S < m.nk) ? k0 + c->S : m.nk;
+  const int kbeg = c->open_k ? 2 : 0, kend = c->open_k ? m.nk - 2 : m.nk;
+  for (int k0 = kbeg; k0 < kend; k0 += c->S) {
+    const int k1 = (k0 + c->S < kend) ? k0 + c->S : kend;
     sl.kbase = (k0 == 0) ? m.nk - 1 : k0 - 1;
     recon(sl.kbase, k1 - k0 + 2);                                   // planes k0-1 .. k1
     launch_flux<CART>(c, sl, Win, dt, sl.kbase, k1 - k0 + 1, stage); // cells of planes k0-1 .. k1-1 own the needed faces
@@ -332,23 +356,58 @@ static void run_stage(cgks_ctx* c, int stage, double dt) {
   }
 }
 
-extern "C" int cgks_step(cgks_ctx* c, double dt) {
-  if (!c || !(dt > 0.0)) return CGKS_EINVAL;
-  for (int stage = 1; stage <= 2; stage++) {
-    if (c->mesh.cart) run_stage<true>(c, stage, dt); else run_stage<false>(c, stage, dt);
-  }
+extern "C" int cgks_stage(cgks_ctx* c, int stage, double dt) {
+  if (!c || !(dt > 0.0) || stage != c->phase + 1) return c ? fail(c, CGKS_EINVAL, "cgks_stage: stages must alternate 1, 2 with dt > 0") : CGKS_EINVAL;
+  if (c->mesh.cart) run_stage<true>(c, stage, dt); else run_stage<false>(c, stage, dt);
   CK(cudaGetLastError());
-  // the saved buffer now holds the state at t_n+1
-  const int old = c->cur; c->cur = c->save; c->save = old;
-  if (c->profiling) { CK(cudaStreamSynchronize(c->stream)); collect_events(c); }
+  if (stage == 1) c->phase = 1;
+  else {      // the saved buffer now holds the state at t_n+1
+    const int old = c->cur; c->cur = c->save; c->save = old;
+    c->phase = 0;
+  }
+  if (c->profiling && stage == 2) { CK(cudaStreamSynchronize(c->stream)); collect_events(c); }
   return CGKS_OK;
 }
+
+extern "C" int cgks_step(cgks_ctx* c, double dt) {
+  if (!c || !(dt > 0.0)) return CGKS_EINVAL;
+  if (c->open_k) return fail(c, CGKS_EINVAL, "cgks_step on a sub-domain: use cgks_stage with a halo exchange before each stage");
+  if (c->phase != 0) return fail(c, CGKS_EINVAL, "cgks_step between cgks_stage 1 and 2");
+  int rc = cgks_stage(c, 1, dt);
+  if (rc == CGKS_OK) rc = cgks_stage(c, 2, dt);
+  return rc;
+}
+
+// ---- sub-domain halos ---------------------------------------------
+extern "C" int cgks_halo_bytes(const cgks_ctx* c, size_t* bytes) {
+  if (!c || !bytes) return CGKS_EINVAL;
+  *bytes = (size_t)NSTATE * 2 * c->mesh.plane * 8;
+  return CGKS_OK;
+}
+
+static int halo_copy(cgks_ctx* c, int side, double* d_buf, bool pack) {
+  if (!c || !d_buf || side < 0 || side > 1) return CGKS_EINVAL;
+  if (!c->open_k) return fail(c, CGKS_EINVAL, "halo calls need a sub-domain context (cgks_create_slab)");
+  const Mesh& m = c->mesh;
+  double* W = c->phase ? c->W[c->star] : c->W[c->cur];
+  // pack: the two outermost OWNED planes of the side; unpack: the two halo planes of the side
+  const int kfirst = pack ? (side ? m.nk - 4 : 2) : (side ? m.nk - 2 : 0);
+  const long tot = (long)NSTATE * 2 * m.plane;
+  long blocks = (tot + 255) / 256; if (blocks > (long)c->nsm * 16) blocks = (long)c->nsm * 16;
+  Timed t(c, KC_OTHER);
+  if (pack) halo_kernel<true><<<(unsigned)blocks, 256, 0, c->stream>>>(W, d_buf, m.n, m.plane, kfirst, 2);
+  else halo_kernel<false><<<(unsigned)blocks, 256, 0, c->stream>>>(W, d_buf, m.n, m.plane, kfirst, 2);
+  return cudaGetLastError() == cudaSuccess ? CGKS_OK : CGKS_ECUDA;
+}
+extern "C" int cgks_pack_halo(cgks_ctx* c, int side, double* d_buf) { return halo_copy(c, side, d_buf, true); }
+extern "C" int cgks_unpack_halo(cgks_ctx* c, int side, const double* d_buf) { return halo_copy(c, side, const_cast<double*>(d_buf), false); }
 
 // ---- test taps: reconstruction / flux of the CURRENT state, whole mesh resident only ------------------------------
 extern "C" int cgks_debug_stage(cgks_ctx* c, double dt, double* d_pv, double* d_fx) {
   if (!c) return CGKS_EINVAL;
   const Mesh& m = c->mesh;
   if (c->S < m.nk) return fail(c, CGKS_ENOMEM, "debug taps need the whole mesh resident");
+  if (c->open_k) return fail(c, CGKS_EINVAL, "debug taps need a whole-mesh context");
   ReconPrm rp{ c->prm.nonlinear, c->prm.geno_C, c->prm.geno_eps, 1.0 / tanh(c->prm.geno_C), c->prm.gamma };
   Slab sl; sl.kbase = 0; sl.slots_pv = c->slots_pv; sl.slots_fx = c->slots_fx;
   sl.stride_pv = (long)c->slots_pv * m.plane; sl.stride_fx = (long)c->slots_fx * m.plane;
@@ -390,6 +449,7 @@ static void run_diagnostics(cgks_ctx* c, double* d_acc) {
 
 extern "C" int cgks_diagnostics(cgks_ctx* c, double* ek_host, double* enstrophy_host) {
   if (!c || !ek_host || !enstrophy_host) return CGKS_EINVAL;
+  if (c->open_k) return fail(c, CGKS_EINVAL, "diagnostics need a whole-mesh context");
   double* d_acc = (double*)((char*)c->d_flags + 40);      // the 24 unused bytes of the 64-byte flags block
   CK(cudaMemsetAsync(d_acc, 0, 3 * sizeof(double), c->stream));
   if (c->mesh.cart) run_diagnostics<true>(c, d_acc); else run_diagnostics<false>(c, d_acc);
@@ -464,6 +524,7 @@ extern "C" int cgks_fp64_peak(void* stream, double* tflops) {
 extern "C" int cgks_run_host(cgks_ctx* c, const double* hQ, const double* hG, const double* hD, double cfl, int nsteps,
                              double* oQ, double* oG, double* oD) {
   if (!c || !hQ || nsteps < 0) return CGKS_EINVAL;
+  if (c->open_k) return fail(c, CGKS_EINVAL, "cgks_run_host needs a whole-mesh context");
   const Mesh& m = c->mesh; const long n = m.n;
   // stage the host arrays through the (currently unused) stage buffer, then run the ordinary set_state path
   double* tmp = c->W[c->star];

@@ -21,12 +21,17 @@ struct NodeView {
 
 // flags[0] |= 1 if any cell's J0 differs from diag(period/n)  (-> general metrics needed)
 // flags[1] |= 1 if det J0 <= 0 or volume <= 0;  flags[2] |= 1 if the node array is not periodic
-__global__ void geometry_kernel(int ni, int nj, int nk, const double* __restrict__ nodes, double* __restrict__ met,
+// The node array is that of the GLOBAL periodic mesh (nk planes of cells); the context holds nkl planes of it starting at
+// global plane kofs (wrapped): nkl = nk, kofs = 0 for a whole-mesh context, a slab with its halo planes for a sub-domain.
+// A cell's metrics are computed from the same eight node values whichever context holds it.
+__global__ void geometry_kernel(int ni, int nj, int nk, int nkl, int kofs, const double* __restrict__ nodes, double* __restrict__ met,
                                 int* __restrict__ flags) {
-  const long n = (long)ni * nj * nk;
+  const long n = (long)ni * nj * nkl;
   const long c = (long)blockIdx.x * blockDim.x + threadIdx.x;
   if (c >= n) return;
-  const int i = (int)(c % ni), j = (int)((c / ni) % nj), k = (int)(c / ((long)ni * nj));
+  const int i = (int)(c % ni), j = (int)((c / ni) % nj);
+  int k = (int)(c / ((long)ni * nj)) + kofs;
+  k %= nk; if (k < 0) k += nk;
   NodeView nv{ nodes, ni + 1, nj + 1, nk + 1 };
   double X[8][3];     // index 4*di + 2*dj + dk
 #pragma unroll
@@ -171,11 +176,13 @@ __global__ void get_state_kernel(Mesh m, const double* __restrict__ W, double* _
 // Warp-shuffle min, one atomicMin per block on the bit pattern (positive doubles order like unsigned integers).
 struct CflPrm { double gamma, mu_ref, omega, T_ref, cfl; };
 
+// Cells of the planes [kA, kA + cnt) only (a sub-domain reduces over the planes it owns).
 __global__ void cfl_kernel(Mesh m, const double* __restrict__ W, CflPrm p, unsigned long long* __restrict__ dt_bits,
-                           int* __restrict__ flag) {
+                           int* __restrict__ flag, int kA, int cnt) {
   double dtmin = INFINITY;
   bool bad = false;
-  for (long c = (long)blockIdx.x * blockDim.x + threadIdx.x; c < m.n; c += (long)gridDim.x * blockDim.x) {
+  const long c0 = (long)kA * m.plane, c1 = c0 + (long)cnt * m.plane;
+  for (long c = c0 + (long)blockIdx.x * blockDim.x + threadIdx.x; c < c1; c += (long)gridDim.x * blockDim.x) {
     const double rho = W[c], mx = W[m.n + c], my = W[2 * m.n + c], mz = W[3 * m.n + c], E = W[4 * m.n + c];
     const double U[3] = { mx / rho, my / rho, mz / rho };
     const double pr = (p.gamma - 1.0) * (E - 0.5 * rho * (U[0] * U[0] + U[1] * U[1] + U[2] * U[2]));
@@ -222,6 +229,19 @@ __global__ void cfl_kernel(Mesh m, const double* __restrict__ W, CflPrm p, unsig
     if (lane == 0) atomicMin(dt_bits, (unsigned long long)__double_as_longlong(dtmin));
   }
   if (bad) atomicOr(flag, 1);
+}
+
+// Halo planes of a sub-domain: `np` k-planes of all 80 state fields between the state
+// buffer W [80][n] and a contiguous buffer [80][np][plane].  PACK: W -> buf, else buf -> W.
+template <bool PACK>
+__global__ void halo_kernel(double* __restrict__ W, double* __restrict__ buf, long n, long plane, int kfirst, int np) {
+  const long per = (long)np * plane;
+  const long tot = (long)NSTATE * per;
+  for (long t = (long)blockIdx.x * blockDim.x + threadIdx.x; t < tot; t += (long)gridDim.x * blockDim.x) {
+    const long f = t / per, r = t - f * per;
+    double* w = W + f * n + (long)kfirst * plane + r;
+    if (PACK) buf[t] = *w; else *w = buf[t];
+  }
 }
 
 }  // namespace cgks
