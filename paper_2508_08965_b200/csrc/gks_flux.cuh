@@ -33,7 +33,7 @@ struct GasConst {
 // Maxwellian (per unit density) and the constants of its primed basis
 struct Maxw {
   double rho, irho, U, V, W, lam, hil;   // hil = 1/(2 lam) = p/rho
-  double sU;                             // U^2 + (K+3)/(2 lam)
+  double hsU;                            // (U^2 + (K+3)/(2 lam))/2
   double c4;                             // 4 lam^2/(K+3)
   double q2;                             // (V^2 + W^2)/2
   double t1;                             // <T> = (K+2)/(2 lam)
@@ -50,7 +50,7 @@ __device__ __forceinline__ void maxw_scalars(Maxw& g, const double* Wc, const Ga
   g.U = Wc[1] * g.irho; g.V = Wc[2] * g.irho; g.W = Wc[3] * g.irho;
   g.hil = 2.0 * gc.inv_K3 * re * (g.irho * g.irho);          // 1/(2 lam) = 2 (rho e)/((K+3) rho) = p/rho
   g.lam = 0.25 * (gc.K + 3.0) * (Wc[0] * Wc[0]) * ire;
-  g.sU = fma(g.U, g.U, (gc.K + 3.0) * g.hil);
+  g.hsU = 0.5 * fma(g.U, g.U, (gc.K + 3.0) * g.hil);
   g.c4 = 4.0 * g.lam * g.lam * gc.inv_K3;
   g.q2 = 0.5 * fma(g.V, g.V, g.W * g.W);
   g.t1 = (gc.K + 2.0) * g.hil;
@@ -73,44 +73,55 @@ __device__ __forceinline__ void mom_recur(double* m, double U, double hil) {
   for (int n = 0; n + 2 < N; n++) m[n + 2] = U * m[n + 1] + (n + 1) * hil * m[n];
 }
 
-// Micro slope in the primed basis, a = (a'_0, a_1, a'_2, a'_3, a_4) with a.psi = a'.psi', from the PRIMED moments
-// hp[alpha] = <(a.psi) psi'_alpha> per unit density (the standard GKS relation with V = W = 0).
+// Micro slope in the primed basis from the PRIMED moments hp[alpha] = <(a.psi) psi'_alpha> per unit density (
+// the standard GKS relation with V = W = 0).  With a.psi = a'.psi', the slope is carried as
+//     a = (a'_0, a_1, a'_2/(2 lam), a'_3/(2 lam), a_4/2):
+// the tangential components only ever appear divided by 2 lam (and then a'_2/(2 lam) = h'_2: no arithmetic at all), and
+// a_4 only halved or times 1/(2 lam).
 __device__ __forceinline__ void micro_slope_primed(const Maxw& g, const double* hp, double* a) {
-  const double R1 = hp[1] - g.U * hp[0];
-  const double R4 = 2.0 * hp[4] - g.sU * hp[0];
-  const double tl = 2.0 * g.lam;
-  a[4] = g.c4 * (R4 - 2.0 * (g.U * R1));
-  a[1] = tl * R1 - g.U * a[4];
-  a[2] = tl * hp[2];
-  a[3] = tl * hp[3];
-  a[0] = hp[0] - g.U * a[1] - 0.5 * (a[4] * g.sU);
+  const double R1 = fma(-g.U, hp[0], hp[1]);
+  const double R4h = fma(-g.hsU, hp[0], hp[4]);                  // (2 h'_4 - (U^2 + (K+3)/(2 lam)) h'_0)/2
+  a[4] = g.c4 * fma(-g.U, R1, R4h);                               // a_4/2 = (4 lam^2/(K+3)) (R_4 - 2 U R_1)/2
+  a[1] = fma(-2.0 * g.U, a[4], (2.0 * g.lam) * R1);
+  a[2] = hp[2];
+  a[3] = hp[3];
+  a[0] = fma(-2.0 * g.hsU, a[4], fma(-g.U, a[1], hp[0]));
 }
 
-// the same from LABORATORY moments h[alpha] = <(a.psi) psi_alpha>: psi' = B^-1 psi first
-__device__ __forceinline__ void micro_slope_lab(const Maxw& g, const double* h, double* a) {
+// the same from LABORATORY moments rho h[alpha] = rho <(a.psi) psi_alpha> (the slope of the conservative variables):
+// psi' = B^-1 psi first, the factor 1/rho applied to the five primed moments
+__device__ __forceinline__ void micro_slope_lab(const Maxw& g, const double* S, double* a) {
   double hp[5];
-  hp[0] = h[0]; hp[1] = h[1];
-  hp[2] = h[2] - g.V * h[0];
-  hp[3] = h[3] - g.W * h[0];
-  hp[4] = h[4] - g.V * hp[2] - g.W * hp[3] - g.q2 * h[0];
+  const double s2 = fma(-g.V, S[0], S[2]), s3 = fma(-g.W, S[0], S[3]);
+  const double s4 = fma(-g.q2, S[0], fma(-g.W, s3, fma(-g.V, s2, S[4])));
+  hp[0] = S[0] * g.irho; hp[1] = S[1] * g.irho; hp[2] = s2 * g.irho; hp[3] = s3 * g.irho; hp[4] = s4 * g.irho;
   micro_slope_primed(g, hp, a);
 }
 
-// out (laboratory basis) += B M (primed moments M)
+// out (laboratory basis) (+)= B M (primed moments M); ACC = false overwrites (the first contribution to a sum)
+template <bool ACC = true>
 __device__ __forceinline__ void lab_acc(const Maxw& g, const double* M, double* out) {
-  out[0] += M[0];
-  out[1] += M[1];
-  out[2] = fma(g.V, M[0], out[2] + M[2]);
-  out[3] = fma(g.W, M[0], out[3] + M[3]);
-  out[4] = fma(g.q2, M[0], fma(g.W, M[3], fma(g.V, M[2], out[4] + M[4])));
+  if (ACC) {
+    out[0] += M[0];
+    out[1] += M[1];
+    out[2] = fma(g.V, M[0], out[2] + M[2]);
+    out[3] = fma(g.W, M[0], out[3] + M[3]);
+    out[4] = fma(g.q2, M[0], fma(g.W, M[3], fma(g.V, M[2], out[4] + M[4])));
+  } else {
+    out[0] = M[0];
+    out[1] = M[1];
+    out[2] = fma(g.V, M[0], M[2]);
+    out[3] = fma(g.W, M[0], M[3]);
+    out[4] = fma(g.q2, M[0], fma(g.W, M[3], fma(g.V, M[2], M[4])));
+  }
 }
 
 // polynomial in u left by a primed slope after the (c_v, c_w, xi) integrals
 struct SlopePoly { double p[3]; double cv, cw, e4; };      // weight 1: p0 + p1 u + p2 u^2; weights c_v, c_w: constants; e4 = a_4/(2 lam)
 
 __device__ __forceinline__ void make_slope_poly(SlopePoly& P, const Maxw& g, const double* a) {
-  P.p[0] = fma(0.5 * a[4], g.t1, a[0]); P.p[1] = a[1]; P.p[2] = 0.5 * a[4];
-  P.cv = a[2] * g.hil; P.cw = a[3] * g.hil; P.e4 = a[4] * g.hil;
+  P.p[0] = fma(a[4], g.t1, a[0]); P.p[1] = a[1]; P.p[2] = a[4];
+  P.cv = a[2]; P.cw = a[3]; P.e4 = (2.0 * g.hil) * a[4];
 }
 
 template <int N>
@@ -145,22 +156,22 @@ __device__ __forceinline__ void apply_slope_QF(const Maxw& g, const SlopePoly& P
 struct DivPoly { double e[4], dv[3], dw[3], g0, g1; };
 
 __device__ __forceinline__ void make_div_poly(DivPoly& D, const Maxw& g, const double* ax, const double* ay, const double* az) {
+  // slopes as carried by micro_slope_primed: (a'_0, a_1, a'_2 h, a'_3 h, a_4/2), h = 1/(2 lam); b = V a_y + W a_z in the same form
   const double h = g.hil;
   double b[5];
 #pragma unroll
   for (int k = 0; k < 5; k++) b[k] = fma(g.V, ay[k], g.W * az[k]);
-  const double tr = ay[2] + az[3];
-  const double hb4 = 0.5 * b[4], hx4 = 0.5 * ax[4];
-  D.e[0] = fma(h, tr, fma(hb4, g.t1, b[0]));
-  D.e[1] = fma(hx4, g.t1, ax[0]) + b[1];
-  D.e[2] = ax[1] + hb4;
-  D.e[3] = hx4;
+  const double htr = ay[2] + az[3];                         // h (a'_y2 + a'_z3)
+  D.e[0] = fma(b[4], g.t1, b[0]) + htr;
+  D.e[1] = fma(ax[4], g.t1, ax[0]) + b[1];
+  D.e[2] = ax[1] + b[4];
+  D.e[3] = ax[4];
   const double t1p = fma(2.0, h, g.t1);                     // <c_v^2 T>/<c_v^2> = (K+4)/(2 lam)
-  const double hy4 = 0.5 * ay[4], hz4 = 0.5 * az[4];
-  D.dv[0] = h * (fma(hy4, t1p, ay[0]) + b[2]); D.dv[1] = h * (ax[2] + ay[1]); D.dv[2] = h * hy4;
-  D.dw[0] = h * (fma(hz4, t1p, az[0]) + b[3]); D.dw[1] = h * (ax[3] + az[1]); D.dw[2] = h * hz4;
-  D.g1 = h * (g.t1 * ax[4]);
-  D.g0 = h * fma(g.t1, b[4], 2.0 * (h * tr));
+  D.dv[0] = fma(h, fma(ay[4], t1p, ay[0]), b[2]); D.dv[1] = fma(h, ay[1], ax[2]); D.dv[2] = h * ay[4];
+  D.dw[0] = fma(h, fma(az[4], t1p, az[0]), b[3]); D.dw[1] = fma(h, az[1], ax[3]); D.dw[2] = h * az[4];
+  const double ht1x2 = 2.0 * (h * g.t1);
+  D.g1 = ht1x2 * ax[4];
+  D.g0 = fma(ht1x2, b[4], 2.0 * (h * htr));
 }
 
 template <int I>
@@ -179,13 +190,22 @@ __device__ __forceinline__ void apply_div_QF(const Maxw& g, const DivPoly& D, co
 }
 
 // out[alpha] (laboratory basis) += <u^I psi_alpha> of the plain Maxwellian with (scaled) u-moments mu
-template <int I>
+template <int I, bool ACC = true>
 __device__ __forceinline__ void add_plain(const Maxw& g, const double* mu, double* out) {
-  out[0] += mu[I];
-  out[1] += mu[I + 1];
-  out[2] = fma(g.V, mu[I], out[2]);
-  out[3] = fma(g.W, mu[I], out[3]);
-  out[4] = fma(fma(0.5, g.t1, g.q2), mu[I], fma(0.5, mu[I + 2], out[4]));
+  const double et = fma(0.5, g.t1, g.q2);
+  if (ACC) {
+    out[0] += mu[I];
+    out[1] += mu[I + 1];
+    out[2] = fma(g.V, mu[I], out[2]);
+    out[3] = fma(g.W, mu[I], out[3]);
+    out[4] = fma(et, mu[I], fma(0.5, mu[I + 2], out[4]));
+  } else {
+    out[0] = mu[I];
+    out[1] = mu[I + 1];
+    out[2] = g.V * mu[I];
+    out[3] = g.W * mu[I];
+    out[4] = fma(et, mu[I], 0.5 * mu[I + 2]);
+  }
 }
 
 struct Groups {        // moments of the groups of Eq. 5 that are shared between both sides (all times rho, laboratory basis)
@@ -196,51 +216,40 @@ struct Groups {        // moments of the groups of Eq. 5 that are shared between
   double G6Q[5], G6F[5];
 };
 
-// one side (left state with the u > 0 half moments, right state with the u < 0 ones)
+// one side (left state with the u > 0 half moments, right state with the u < 0 ones); ACC = false: the first side, which
+// initialises the sums over both sides
+template <bool ACC>
 __device__ __forceinline__ void gks_side(const Maxw& g, double mh0, double mh1, const double (*S)[5], Groups& G, double* dQs) {
   double mu[6], mh[7];
   mu[0] = 1.0; mu[1] = g.U; mom_recur<6>(mu, g.U, g.hil);
   mh[0] = mh0; mh[1] = mh1;                      // half-space moments, pre-scaled by rho
   mom_recur<7>(mh, g.U, g.hil);
-  add_plain<0>(g, mh, G.W0);
-  add_plain<1>(g, mh, G.G4F);
+  add_plain<0, ACC>(g, mh, G.W0);
+  add_plain<1, ACC>(g, mh, G.G4F);
   // micro slopes of the one-sided Maxwellian (primed basis); their half-space moments feed the slopes of W0
-  double a[3][5], h[5], M[5], MF[5];
+  double a[3][5], M[5], MF[5];
 #pragma unroll
   for (int d = 0; d < 3; d++) {
-#pragma unroll
-    for (int v = 0; v < 5; v++) h[v] = S[d][v] * g.irho;
-    micro_slope_lab(g, h, a[d]);
+    micro_slope_lab(g, S[d], a[d]);
     SlopePoly P; make_slope_poly(P, g, a[d]);
     apply_slope<0>(g, P, mh, M);
-    lab_acc(g, M, G.dW0[d]);
+    lab_acc<ACC>(g, M, G.dW0[d]);
   }
   DivPoly D; make_div_poly(D, g, a[0], a[1], a[2]);
   // time slope from the compatibility condition <a_x u + a_y v + a_z w + A> = 0 (full velocity space): the primed
   // moments go straight into the primed solve
   apply_div<0>(g, D, mu, M);
 #pragma unroll
-  for (int v = 0; v < 5; v++) { M[v] = -M[v]; dQs[v] = 0.0; }
-  lab_acc(g, M, dQs);
+  for (int v = 0; v < 5; v++) M[v] = -M[v];
+  lab_acc<false>(g, M, dQs);
 #pragma unroll
   for (int v = 0; v < 5; v++) dQs[v] *= g.rho;                                // d/dt of the one-sided Maxwellian's moments
   double A[5]; micro_slope_primed(g, M, A);
   apply_div_QF(g, D, mh, M, MF);
-  lab_acc(g, M, G.G5Q); lab_acc(g, MF, G.G5F);
+  lab_acc<ACC>(g, M, G.G5Q); lab_acc<ACC>(g, MF, G.G5F);
   SlopePoly PA; make_slope_poly(PA, g, A);
   apply_slope_QF(g, PA, mh, M, MF);
-  lab_acc(g, M, G.G6Q); lab_acc(g, MF, G.G6F);
-}
-
-// time-integrated coefficients of the six groups of Eq. 5 over [0,T]
-__device__ __forceinline__ void time_coef(double T, double tau, double E, double* cf) {
-  const double ome = 1.0 - E;
-  cf[0] = T - tau * ome;
-  cf[1] = 2.0 * tau * tau * ome - tau * T * (1.0 + E);
-  cf[2] = 0.5 * T * T - tau * T + tau * tau * ome;
-  cf[3] = tau * ome;
-  cf[4] = tau * T * E - 2.0 * tau * tau * ome;
-  cf[5] = -tau * tau * ome;
+  lab_acc<ACC>(g, M, G.G6Q); lab_acc<ACC>(g, MF, G.G6F);
 }
 
 // Full solver in the face frame.  WL/WR[5] and SL/SR[3][5] are the rotated states and (n, t1, t2) slopes.
@@ -250,11 +259,6 @@ __device__ __forceinline__ void gks_flux_local(const GasConst& gc, double dt, do
                                                const double* WR, const double (*SR)[5],
                                                double* Fn, double* Ft, double* VL, double* DL, double* VR, double* DR) {
   Groups G;
-#pragma unroll
-  for (int v = 0; v < 5; v++) {
-    G.W0[v] = 0; G.G4F[v] = 0; G.G5Q[v] = 0; G.G5F[v] = 0; G.G6Q[v] = 0; G.G6F[v] = 0;
-    G.dW0[0][v] = 0; G.dW0[1][v] = 0; G.dW0[2][v] = 0;
-  }
   // scalars and half-space moments of both sides first: the two erfc/exp/sqrt/reciprocal chains are independent and
   // overlap in the FP64 pipe; the slopes of each side follow
   double pl, pr;
@@ -264,33 +268,31 @@ __device__ __forceinline__ void gks_flux_local(const GasConst& gc, double dt, do
     maxw_scalars(gl, WL, gc); maxw_scalars(gr, WR, gc);
     half_moments(gl, 1.0, hl0, hl1); half_moments(gr, -1.0, hr0, hr1);
     pl = gl.rho * gl.hil; pr = gr.rho * gr.hil;
-    gks_side(gl, hl0, hl1, SL, G, DL);     // DL, DR hold the one-sided time derivatives for now
-    gks_side(gr, hr0, hr1, SR, G, DR);
+    gks_side<false>(gl, hl0, hl1, SL, G, DL);     // DL, DR hold the one-sided time derivatives for now
+    gks_side<true>(gr, hr0, hr1, SR, G, DR);
   }
   // equilibrium state g0 and its slopes
   Maxw g0; maxw_scalars(g0, G.W0, gc);
   double mu[7];
   mu[0] = g0.rho; mu[1] = g0.rho * g0.U; mom_recur<7>(mu, g0.U, g0.hil);     // full moments times rho0
-  double G1F[5] = { 0, 0, 0, 0, 0 }, G2Q[5] = { 0, 0, 0, 0, 0 }, G2F[5] = { 0, 0, 0, 0, 0 }, G3F[5] = { 0, 0, 0, 0, 0 };
-  add_plain<1>(g0, mu, G1F);
+  double G1F[5], G2Q[5], G2F[5], G3F[5];
+  add_plain<1, false>(g0, mu, G1F);
   {
     double a[3][5], h[5], MQ[5], MF[5];
 #pragma unroll
     for (int d = 0; d < 3; d++) {
-#pragma unroll
-      for (int v = 0; v < 5; v++) h[v] = G.dW0[d][v] * g0.irho;
-      micro_slope_lab(g0, h, a[d]);
+      micro_slope_lab(g0, G.dW0[d], a[d]);
     }
     DivPoly D; make_div_poly(D, g0, a[0], a[1], a[2]);
     apply_div_QF(g0, D, mu, MQ, MF);
-    lab_acc(g0, MQ, G2Q); lab_acc(g0, MF, G2F);
+    lab_acc<false>(g0, MQ, G2Q); lab_acc<false>(g0, MF, G2F);
     // Abar from <abar.u + Abar> = 0: its primed conserved moments are -MQ
 #pragma unroll
     for (int v = 0; v < 5; v++) h[v] = -MQ[v] * g0.irho;
     double A[5]; micro_slope_primed(g0, h, A);
     SlopePoly PA; make_slope_poly(PA, g0, A);
     apply_slope<1>(g0, PA, mu, MF);
-    lab_acc(g0, MF, G3F);
+    lab_acc<false>(g0, MF, G3F);
   }
   // collision time
   double tau_phys = 0.0;
@@ -301,26 +303,30 @@ __device__ __forceinline__ void gks_flux_local(const GasConst& gc, double dt, do
   }
   const double dpr = ddiv(fabs(pl - pr), fabs(pl + pr));
   const double tau = tau_phys + gc.c1 * dt + gc.c2 * dpr * dt;
-  double c1[6], c2[6];
-  if (tau == 0.0) {     // reading T2: f = g0 (1 + Abar t)
-    c1[0] = dt; c1[1] = 0; c1[2] = 0.5 * dt * dt; c1[3] = c1[4] = c1[5] = 0;
-    c2[0] = 0.5 * dt; c2[1] = 0; c2[2] = 0.125 * dt * dt; c2[3] = c2[4] = c2[5] = 0;
-  } else {
-    const double E2 = dexp(-0.5 * dt * drcp(tau)), E1 = E2 * E2;
-    time_coef(dt, tau, E1, c1); time_coef(0.5 * dt, tau, E2, c2);
+  // Time-integrated coefficients of the six groups of Eq. 5 over [0, dt] and [0, dt/2], combined as
+  // f^n = (4 fbar(dt/2) - fbar(dt))/dt and f_t^n = 4 (fbar(dt) - 2 fbar(dt/2))/dt^2, in closed form: with
+  // E = exp(-dt/(2 tau)), x = 1 - E, y = tau/dt, w = 4 y x^2/dt, u = 4 y E x, z = y x (3 - E), s = E (2 - E)
+  //   c_t = [ w, u - 2 tau w, 1 - tau w, -w, 2 tau w - u, tau w ]           (so the W0 coefficient c_t0 + c_t3 vanishes)
+  //   c_n = [ 1 - z, tau (2z - s - 1), -tau (1 - z), z, tau (s - 2z), -tau z ]   (and c_n0 + c_n3 = 1)
+  // which avoids the cancellation between the two time integrals.  tau = 0 (reading T2): f = g0 (1 + Abar t).
+  double cn[6] = { 1.0, 0.0, 0.0, 0.0, 0.0, 0.0 }, ct[6] = { 0.0, 0.0, 1.0, 0.0, 0.0, 0.0 };
+  if (tau != 0.0) {
+    const double E = dexp(-0.5 * dt * drcp(tau)), x = 1.0 - E, y = tau * idt;
+    const double w = 4.0 * (y * idt) * (x * x), u = 4.0 * y * (E * x), tw = tau * w;
+    ct[0] = w; ct[1] = u - 2.0 * tw; ct[2] = 1.0 - tw; ct[3] = -w; ct[4] = -ct[1]; ct[5] = tw;
+    if (!STAGE2) {
+      const double z = y * x * (3.0 - E), sE = E * (2.0 - E);
+      cn[0] = 1.0 - z; cn[1] = tau * (2.0 * z - sE - 1.0); cn[2] = -tau * cn[0]; cn[3] = z; cn[4] = tau * (sE - 2.0 * z); cn[5] = -tau * z;
+    }
   }
-  // f^n = (4 fbar(dt/2) - fbar(dt))/dt,  f_t^n = 4 (fbar(dt) - 2 fbar(dt/2))/dt^2
-  double cn[6], ct[6];
-#pragma unroll
-  for (int q = 0; q < 6; q++) { cn[q] = (4.0 * c2[q] - c1[q]) * idt; ct[q] = 4.0 * (c1[q] - 2.0 * c2[q]) * idt * idt; }
   double Qn[5], Qt[5];
-  const double cnW = cn[0] + cn[3], cnG = cn[1] - cn[2], ctW = ct[0] + ct[3], ctG = ct[1] - ct[2];
+  const double cnG = cn[1] - cn[2], ctG = ct[1] - ct[2];       // the conserved moments of group 3 are minus those of group 2
 #pragma unroll
   for (int v = 0; v < 5; v++) {
-    Qt[v] = ctW * G.W0[v] + ctG * G2Q[v] + ct[4] * G.G5Q[v] + ct[5] * G.G6Q[v];
+    Qt[v] = ctG * G2Q[v] + ct[4] * G.G5Q[v] + ct[5] * G.G6Q[v];
     Ft[v] = ct[0] * G1F[v] + ct[1] * G2F[v] + ct[2] * G3F[v] + ct[3] * G.G4F[v] + ct[4] * G.G5F[v] + ct[5] * G.G6F[v];
     if (!STAGE2) {
-      Qn[v] = cnW * G.W0[v] + cnG * G2Q[v] + cn[4] * G.G5Q[v] + cn[5] * G.G6Q[v];
+      Qn[v] = G.W0[v] + cnG * G2Q[v] + cn[4] * G.G5Q[v] + cn[5] * G.G6Q[v];
       Fn[v] = cn[0] * G1F[v] + cn[1] * G2F[v] + cn[2] * G3F[v] + cn[3] * G.G4F[v] + cn[4] * G.G5F[v] + cn[5] * G.G6F[v];
     }
   }
