@@ -105,6 +105,20 @@ int cgks_halo_bytes(const cgks_ctx*, size_t* bytes);
 int cgks_pack_halo(cgks_ctx*, int side, double* d_buf);
 int cgks_unpack_halo(cgks_ctx*, int side, const double* d_buf);
 
+/* Non-periodic boundary in k: instead of a neighbour's planes, the two halo planes of `side` of a
+   sub-domain context are filled by a boundary rule applied to the owned planes of the stage's input state (call it before
+   each stage, like the halo exchange).  The paper names its boundary types (no-slip adiabatic wall and far field,
+   PAPER.md:494; non-reflecting) without formulas; reading B1:
+     CGKS_BC_SLIP_WALL   mirror image about the boundary face, normal momentum odd (slip wall = symmetry plane)
+     CGKS_BC_NOSLIP_WALL mirror image, all momentum components odd: zero velocity and zero normal temperature gradient at
+                         the face (no-slip adiabatic wall)
+     CGKS_BC_OUTFLOW     zero-gradient extrapolation of the outermost owned plane
+     CGKS_BC_FARFIELD    the uniform state far_state_host[5] (host pointer: rho, rho U, rho V, rho W, rho E)
+   Uniform Cartesian meshes only (CGKS_EINVAL otherwise).  A domain bounded in k on both sides is the sub-domain
+   cgks_create_slab(..., k0 = 0, nk_owned = nk_global, ...) with this call on both sides. */
+enum { CGKS_BC_SLIP_WALL = 0, CGKS_BC_NOSLIP_WALL = 1, CGKS_BC_OUTFLOW = 2, CGKS_BC_FARFIELD = 3 };
+int cgks_fill_halo_bc(cgks_ctx*, int side, int kind, const double* far_state_host);
+
 /* Diagnostics of the current state: volume-averaged kinetic energy E_k = int rho |U|^2/2 dV / |Omega| and
    enstrophy int mu |curl U|^2 dV / |Omega| (rho_0 = 1), by the 2x2x2 Gauss rule on every cell with values and velocity
    derivatives from the compact reconstruction (the scheme's own polynomial, Eq. 16; reading X1); mu is the

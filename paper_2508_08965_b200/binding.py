@@ -12,6 +12,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libcgks.so")
 
 CGKS_OK, CGKS_EINVAL, CGKS_ENOMEM, CGKS_ECUDA, CGKS_ENONPHYSICAL = 0, -1, -2, -3, -4
+BC_SLIP_WALL, BC_NOSLIP_WALL, BC_OUTFLOW, BC_FARFIELD = 0, 1, 2, 3
 KERNEL_CLASSES = {"recon": 0, "flux": 1, "update": 2, "cfl": 3, "other": 4}
 
 
@@ -51,6 +52,7 @@ def lib():
         L.cgks_halo_bytes.argtypes = [_vp, C.POINTER(C.c_size_t)]
         L.cgks_pack_halo.argtypes = [_vp, C.c_int, _vp]
         L.cgks_unpack_halo.argtypes = [_vp, C.c_int, _vp]
+        L.cgks_fill_halo_bc.argtypes = [_vp, C.c_int, C.c_int, C.POINTER(C.c_double)]
         L.cgks_status.argtypes = [_vp]
         L.cgks_diagnostics.argtypes = [_vp, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.cgks_run_host.argtypes = [_vp, _vp, _vp, _vp, C.c_double, C.c_int, _vp, _vp, _vp]
@@ -202,6 +204,17 @@ class Solver:
 
     def unpack_halo(self, side, buf):
         self._check(lib().cgks_unpack_halo(self._h, int(side), _ptr(buf)))
+
+    def fill_halo_bc(self, side, kind, far_state=None):
+        """cgks_fill_halo_bc: boundary rule `kind` (BC_*) for the halo planes of `side`; far_state = 5 conservative values."""
+        far = None if far_state is None else (C.c_double * 5)(*[float(x) for x in far_state])
+        self._check(lib().cgks_fill_halo_bc(self._h, int(side), int(kind), far))
+
+    def step_bounded(self, dt, bc_lo, bc_hi, far_state=None):
+        """One S2O4 step of a sub-domain bounded in k on both sides: the boundary rules before each stage, then the stage."""
+        for stage in (1, 2):
+            self.fill_halo_bc(0, bc_lo, far_state); self.fill_halo_bc(1, bc_hi, far_state)
+            self.stage(stage, dt)
 
     def diagnostics(self):
         """(E_k, enstrophy) of the current state, divided by |Omega|."""

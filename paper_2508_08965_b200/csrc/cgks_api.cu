@@ -399,6 +399,19 @@ static int halo_copy(cgks_ctx* c, int side, double* d_buf, bool pack) {
   else halo_kernel<false><<<(unsigned)blocks, 256, 0, c->stream>>>(W, d_buf, m.n, m.plane, kfirst, 2);
   return cudaGetLastError() == cudaSuccess ? CGKS_OK : CGKS_ECUDA;
 }
+extern "C" int cgks_fill_halo_bc(cgks_ctx* c, int side, int kind, const double* far_state_host) {
+  if (!c || side < 0 || side > 1 || kind < 0 || kind > 3) return CGKS_EINVAL;
+  if (!c->open_k) return fail(c, CGKS_EINVAL, "halo calls need a sub-domain context (cgks_create_slab)");
+  if (!c->mesh.cart) return fail(c, CGKS_EINVAL, "boundary conditions in k need a uniform Cartesian mesh");
+  if (kind == 3 && !far_state_host) return fail(c, CGKS_EINVAL, "far-field boundary needs a state");
+  const Mesh& m = c->mesh;
+  BcPrm bc; bc.side = side; bc.kind = kind;
+  for (int v = 0; v < 5; v++) bc.far[v] = far_state_host ? far_state_host[v] : 0.0;
+  double* W = c->phase ? c->W[c->star] : c->W[c->cur];
+  Timed t(c, KC_OTHER);
+  bc_halo_kernel<<<dim3((unsigned)((m.plane + 127) / 128), NSTATE, 2), 128, 0, c->stream>>>(W, m.n, m.plane, m.nk, bc);
+  return cudaGetLastError() == cudaSuccess ? CGKS_OK : CGKS_ECUDA;
+}
 extern "C" int cgks_pack_halo(cgks_ctx* c, int side, double* d_buf) { return halo_copy(c, side, d_buf, true); }
 extern "C" int cgks_unpack_halo(cgks_ctx* c, int side, const double* d_buf) { return halo_copy(c, side, const_cast<double*>(d_buf), false); }
 

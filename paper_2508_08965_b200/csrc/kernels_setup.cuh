@@ -244,4 +244,43 @@ __global__ void halo_kernel(double* __restrict__ W, double* __restrict__ buf, lo
   }
 }
 
+// Boundary conditions in k for a sub-domain context (the paper names its boundary types, PAPER.md:494
+// and 536, without formulas: DESIGN.md reading B1): the two halo planes of one side are filled from the owned planes.
+//   kind 0 slip wall / symmetry plane: mirror image about the boundary face; the normal momentum is odd, everything else even
+//   kind 1 no-slip adiabatic wall: mirror image with ALL momentum components odd (zero velocity, zero normal
+//          temperature gradient at the face)
+//   kind 2 outflow: the outermost owned plane copied into both halo planes with its k-derivative dof set to zero
+//   kind 3 far field: a given uniform state, zero derivative dof
+// Mirror rules for the derivative dof of a field of parity s: G_r -> s G_r (r = i, j), -s G_k; line differences along i or j
+// swap the two lines that differ in their k position (index bit b) with sign s; line differences along k keep their
+// index and get the sign -s.  Uniform Cartesian meshes only (the halo cells' metrics are those of the periodic image).
+struct BcPrm { int side, kind; double far[5]; };
+
+__global__ void bc_halo_kernel(double* __restrict__ W, long n, long plane, int nkl, BcPrm bc) {
+  const long ij = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (ij >= plane) return;
+  const int f = blockIdx.y, hp = blockIdx.z;             // field 0..79, halo plane 0 (next to the boundary) or 1
+  const int kt = bc.side ? nkl - 2 + hp : 1 - hp;
+  int ks = bc.side ? nkl - 3 - hp : 2 + hp;              // mirror image
+  if (bc.kind == 2) ks = bc.side ? nkl - 3 : 2;
+  int v, fs = f; double sgn = 1.0; bool kderiv = false;
+  if (f < 5) v = f;
+  else if (f < 20) { v = (f - 5) / 3; const int r = (f - 5) % 3; kderiv = (r == 2); if (r == 2) sgn = -1.0; }
+  else {
+    v = (f - 20) / 12; const int s_ = (f - 20) % 12, ax = s_ / 4;
+    if (ax == 2) { sgn = -1.0; kderiv = true; }
+    else fs = 20 + 12 * v + (s_ ^ 1);                    // bit b = position along the second other axis = k for lines along i or j
+  }
+  double out;
+  if (bc.kind <= 1) {
+    const bool odd = (v == 3) || (bc.kind == 1 && (v == 1 || v == 2));
+    out = (odd ? -sgn : sgn) * W[(long)fs * n + (long)ks * plane + ij];
+  } else if (bc.kind == 2) {
+    out = kderiv ? 0.0 : W[(long)f * n + (long)ks * plane + ij];
+  } else {
+    out = (f < 5) ? bc.far[f] : 0.0;
+  }
+  W[(long)f * n + (long)kt * plane + ij] = out;
+}
+
 }  // namespace cgks
