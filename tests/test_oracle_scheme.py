@@ -138,19 +138,32 @@ def test_axis_permutation_symmetry_of_a_step():
 
 # ----------------------------------------------------------------------------- P4/P5/P6: Tables 1 and 2
 def test_P4_table1_linear_and_order():
-    """Table 1: linear CGKS-5, t = 2.  The oracle's readings reproduce the printed errors to
-    within 5 % (10^3) / 8 % (20^3) and the printed order (4.94) to within 0.2."""
+    """Table 1: linear CGKS-5, t = 2.  With the readings taken the oracle's errors are within
+    -3.7 / -0.7 % (10^3) and +6.7 / +6.6 % (20^3) of the printed L1 / L2 values: the closest of the readings compared by
+    oracle/readings_table.py, and the printed order (4.94) is matched to within 0.2."""
     gold = golden()
     l1_10, l2_10, Q0, Q1 = run_sine(10, 0)
     l1_20, l2_20, _, _ = run_sine(20, 0)
-    assert abs(l1_10 / gold[(1, 10)][0] - 1) < 0.05 and abs(l2_10 / gold[(1, 10)][1] - 1) < 0.05
-    assert abs(l1_20 / gold[(1, 20)][0] - 1) < 0.08 and abs(l2_20 / gold[(1, 20)][1] - 1) < 0.08
+    assert abs(l1_10 / gold[(1, 10)][0] - 1) < 0.045 and abs(l2_10 / gold[(1, 10)][1] - 1) < 0.015
+    assert abs(l1_20 / gold[(1, 20)][0] - 1) < 0.075 and abs(l2_20 / gold[(1, 20)][1] - 1) < 0.075
     order = math.log2(l1_10 / l1_20)
     assert abs(order - 4.9415) < 0.2, order
     # the printed L1/L2 ratio (2.58 at 10^3) fixes the norm definition (reading T3)
     assert abs(l1_10 / l2_10 - gold[(1, 10)][0] / gold[(1, 10)][1]) < 0.1
     # conservation over the whole run
     np.testing.assert_allclose(Q1.sum(axis=(1, 2, 3)), Q0.sum(axis=(1, 2, 3)), rtol=1e-13)
+
+
+def test_P4b_table1_to_one_percent_with_half_the_time_step():
+    """The remaining deviation of P4 is TEMPORAL: with half the time step (CFL 0.25 in reading S3) the oracle reproduces
+    Table 1 at 20^3 to +0.7 % (L1) / +0.2 % (L2) and the 10^3 L2 value to +0.4 % (oracle/readings_table.py).  The spatial
+    operator -- stencil, Eq. 14/19 rows, row scalings, tau_2 normalisation (R4, R5), the tau = 0 flux and the norms (T3) --
+    is therefore the authors'; what differs is the size of their time step, which the paper does not give (S3)."""
+    gold = golden()
+    l1, l2, _, _ = run_sine(20, 0, cfl=0.25)
+    assert abs(l1 / gold[(1, 20)][0] - 1) < 0.015 and abs(l2 / gold[(1, 20)][1] - 1) < 0.01, (l1, l2)
+    l1, l2, _, _ = run_sine(10, 0, cfl=0.25)
+    assert abs(l1 / gold[(1, 10)][0] - 1) < 0.05 and abs(l2 / gold[(1, 10)][1] - 1) < 0.01, (l1, l2)
 
 
 def test_P6_table2_pattern():
