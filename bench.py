@@ -36,6 +36,7 @@ UNIT = "cell-updates/s"
 #    a fraction formed with it exceeds 1; it is printed beside the other, not used as the numerator.
 FLUX_FLOPS_STAGE1 = 2176.0          # 820.4 DFMA + 443.8 DMUL + 91.3 DADD per point
 FLUX_FLOPS_STAGE2 = 2025.0          # 758.5 DFMA + 422.8 DMUL + 85.3 DADD per point
+FLUX_SOURCE_SHA16 = "e8b455be08183f62"      # sha256 (16 hex digits) of gks_flux.cuh + fastmath64.cuh + math_gen.cuh the counts were taken on
 FLUX_FLOPS_ORACLE = 15584.0          # tests/test_abi.py checks this constant against oracle/flop_count.py
 # Round 1's kernel executed 3092.7 / 2923.2 flops per point for the same result (profiles/r01d_kernels_128.md); VERDICT r1's
 # target "frac >= 0.50, i.e. flux <= 223 ms per step" is stated in that count, so the fraction in that count is printed too.
@@ -261,7 +262,10 @@ def run_ours(args):
         nb = int(Qhost.numel() * 8)
         e2e = {"value": cells_job * args.steps / float(te.item()), "unit": UNIT,
                "h2d_bytes_per_step": nb, "d2h_bytes_per_step": nb,
-               "note": "every bench step ships the 5 cell-average fields (Q) host->device from pinned memory through cgks_run_host, "
+               "note": ("slab mode: every bench step ships this rank's slab of Q (with its halo planes) host->device from pinned memory, "
+                        "calls cgks_set_state, one full S2O4 step with the halo exchanges, cgks_get_state, and ships Q back; G and D are "
+                        "re-bootstrapped on the device (reading S2)") if use_slab else
+                       "every bench step ships the 5 cell-average fields (Q) host->device from pinned memory through cgks_run_host, "
                        "runs one full S2O4 step and ships Q back; the 75 derivative dof per cell (G, D) are NOT shipped: they are "
                        "re-bootstrapped from Q on the device (DESIGN.md reading S2) and not returned, so this is a cold-start step "
                        "(the full 80-dof state would be 36.2 GB each way at 384^3, i.e. PCIe-bound at ~1.5 s per step)"}

@@ -260,3 +260,35 @@ def test_positivity_fallback_fires_by_an_O1_margin_and_stays_conservative(name):
     np.testing.assert_allclose(Q1.sum(axis=(1, 2, 3)), tot0, rtol=1e-13, atol=1e-12)
     assert Q1[0].min() > 0
     s.close()
+
+
+# ----------------------------------------------------------------------------- GENO weights on worked examples
+def test_geno_formulas_on_worked_examples():
+    """The blending formulas as the paper prints them, evaluated BY HAND on data for which every ingredient has a closed form.
+    (i) omega_m = (d_m/(IS_m + eps)^5)/sum: face-neighbour differences g_m with all line differences zero
+    give b^m = +-g_m e_axis, IS_m = g_m^2, so omega_0/omega_1 = ((g_1^2 + eps)/(g_0^2 + eps))^5: the exponent 5 and the
+    normalisation.  (ii) chi for the 1-D polynomial P = a xi + c xi^3 (reproduced exactly by the quartic): by hand
+    int P'^2 = a^2 + a c/2 + 9 c^2/80, int P''^2 = 3 c^2, int P'''^2 = 36 c^2, so IS^L, IS^H and (reading G2) IS^tau are known
+    numbers; alpha^{H,L} = 1 + (IS^tau/(IS^{H,L} + eps))^2, alpha = 2 alpha^H/(alpha^H + alpha^L), chi = tanh(C alpha)/tanh C
+    (C = 5 by reading G3): the exponent r = 2, the roles of H and L, the tanh map."""
+    from tests import refdata as rd
+    from tests.test_oracle_recon import NL
+    g = np.array([0.3, -0.5, 0.2, 0.7, -0.4, 0.25])
+    d = np.zeros(72); d[:6] = g
+    _, b, _, om, _, _ = ref.recon_reference(NL, d)
+    eps = 1e-15
+    for m in range(6):
+        assert abs(np.abs(b[m]).sum() - abs(g[m])) < 1e-15                  # b^m = +-g_m along the face normal only
+    w = (1.0 / 6.0) / (g ** 2 + eps) ** 5
+    np.testing.assert_allclose(om, w / w.sum(), rtol=1e-12)
+    assert abs(om[0] / om[1] - ((g[1] ** 2 + eps) / (g[0] ** 2 + eps)) ** 5) < 1e-10 * om[0] / om[1]
+    for a_, c_ in ((1.0, 0.5), (0.2, 1.5), (1.0, 0.01)):
+        fn, grad = rd.poly_fn({(1, 0, 0): a_, (3, 0, 0): c_})
+        _, d = rd.data_vector(fn, grad)
+        _, _, chi, _, _, _ = ref.recon_reference(NL, d)
+        is1 = a_ * a_ + a_ * c_ / 2.0 + 9.0 * c_ * c_ / 80.0; is2 = 3.0 * c_ * c_; is3 = 36.0 * c_ * c_
+        ish = is1 + is2 + is3; ist = is3
+        ah = 1.0 + (ist / (ish + eps)) ** 2; al = 1.0 + (ist / (is1 + eps)) ** 2
+        alpha = 2.0 * ah / (ah + al)
+        assert abs(chi - math.tanh(5.0 * alpha) / math.tanh(5.0)) < 1e-11, (a_, c_, chi)
+    assert chi > 0.999                                                       # nearly linear data: the quartic is kept
