@@ -551,10 +551,12 @@ extern "C" int cgks_run_host(cgks_ctx* c, const double* hQ, const double* hG, co
     rc = cgks_compute_dt(c, cfl, &dt); if (rc) return rc;
     rc = cgks_step(c, dt); if (rc) return rc;
   }
-  const double* Wc = c->W[c->cur];      // state layout equals the user layout: Q | G | D
-  if (oQ) CK(cudaMemcpyAsync(oQ, Wc, (size_t)5 * n * 8, cudaMemcpyDeviceToHost, c->stream));
-  if (oG) CK(cudaMemcpyAsync(oG, Wc + 5 * n, (size_t)15 * n * 8, cudaMemcpyDeviceToHost, c->stream));
-  if (oD) CK(cudaMemcpyAsync(oD, Wc + 20 * n, (size_t)60 * n * 8, cudaMemcpyDeviceToHost, c->stream));
+  // the internal record layout differs from the user layout Q | G | D: stage the output through the (now free) stage buffer
+  rc = cgks_get_state(c, oQ ? tmp : nullptr, oG ? tmp + 5 * n : nullptr, oD ? tmp + 20 * n : nullptr);
+  if (rc) return rc;
+  if (oQ) CK(cudaMemcpyAsync(oQ, tmp, (size_t)5 * n * 8, cudaMemcpyDeviceToHost, c->stream));
+  if (oG) CK(cudaMemcpyAsync(oG, tmp + 5 * n, (size_t)15 * n * 8, cudaMemcpyDeviceToHost, c->stream));
+  if (oD) CK(cudaMemcpyAsync(oD, tmp + 20 * n, (size_t)60 * n * 8, cudaMemcpyDeviceToHost, c->stream));
   return cgks_status(c);
 }
 

@@ -6,15 +6,24 @@
 namespace cgks {
 
 // ---- HBM layout (all fp64, structure-of-arrays, i fastest) ---------------------------------------------------------
-// state buffer        [80][N]      planes: Q v (0..4) | G 5+3v+r (5..19) | D 20+12v+s (20..79)
+// state buffer        80 N doubles: [5][N][4] records { Q_v, G_v (3) } (32 B), then [5][N][12] records D_v (96 B).  A neighbour's
+//                     average and gradient arrive with ONE 256-bit load (one 32-byte sector), a cell's 12 line differences with
+//                     three, and the update writes them with as many stores: 22 loads per (cell, variable) in the
+//                     reconstruction instead of 85 with one plane per component.
 // metrics (general)   [37][N]      J0 3r+a (0..8) | J0^-1 9+3a+r... see MET_* | vol | +face vector areas | +face tangents
 // pv (slab)           [24*5][slots*plane][4]   record (point p = 4m+q, variable v, cell slot) = { value, physical gradient (3) }
 // fx (slab)           [360][slots*plane]   plane (4ax+q)*30 + c : Fn 0..4 | Ft 5..9 | VL 10..14 | DL 15..19 | VR 20..24 | DR 25..29
 enum { NVAR = 5, NSTATE = 80, NPV = 480, NFX = 360, NMET = 37 };
 enum { MET_J0 = 0, MET_J0INV = 9, MET_VOL = 18, MET_AREA = 19, MET_TAN = 28 };
-__host__ __device__ inline int planeQ(int v) { return v; }
-__host__ __device__ inline int planeG(int v, int r) { return 5 + 3 * v + r; }
-__host__ __device__ inline int planeD(int v, int s) { return 20 + 12 * v + s; }
+// index of the first double of the records of (variable v, cell c) in a state buffer of n cells
+__host__ __device__ inline long iQG(int v, long c, long n) { return ((long)v * n + c) * 4; }             // + 0: Q, + 1 + r: G_r
+__host__ __device__ inline long iD(int v, long c, long n) { return 20 * n + ((long)v * n + c) * 12; }   // + s: D_s
+// field number f = 0..79 in the user order (Q v | G 5+3v+r | D 20+12v+s) -> index in the state buffer
+__host__ __device__ inline long iField(int f, long c, long n) {
+  if (f < 5) return iQG(f, c, n);
+  if (f < 20) return iQG((f - 5) / 3, c, n) + 1 + (f - 5) % 3;
+  return iD((f - 20) / 12, c, n) + (f - 20) % 12;
+}
 
 struct Mesh {
   int ni, nj, nk;
@@ -41,6 +50,19 @@ __device__ __forceinline__ bool admissible(const double* w) {
   const double m2 = __dadd_rn(__dadd_rn(__dmul_rn(w[1], w[1]), __dmul_rn(w[2], w[2])), __dmul_rn(w[3], w[3]));
   const double re = __dsub_rn(__dmul_rn(w[0], w[4]), __dmul_rn(0.5, m2));
   return (w[0] > 0.0) && (re > 0.0);
+}
+
+// 256-bit global loads / stores of four consecutive doubles (32-byte aligned)
+__device__ __forceinline__ void ld4(const double* p, double& a, double& b, double& c, double& d) {
+  asm volatile("ld.global.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(a), "=d"(b), "=d"(c), "=d"(d) : "l"(__cvta_generic_to_global(p)) : "memory");
+}
+__device__ __forceinline__ void st4(double* p, double a, double b, double c, double d) {
+  asm volatile("st.global.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(__cvta_generic_to_global(p)), "d"(a), "d"(b), "d"(c), "d"(d) : "memory");
+}
+
+// the same load from data the kernel never writes: non-coherent path, free for the compiler to schedule
+__device__ __forceinline__ void ld4_ro(const double* p, double& a, double& b, double& c, double& d) {
+  asm("ld.global.nc.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(a), "=d"(b), "=d"(c), "=d"(d) : "l"(__cvta_generic_to_global(p)));
 }
 
 struct CellIdx { int i, j, k; long ij; long c; };

@@ -131,7 +131,9 @@ __global__ void set_state_kernel(Mesh m, const double* __restrict__ Qin, const d
   const int v = blockIdx.y;
   const int i = (int)(c % m.ni), j = (int)((c / m.ni) % m.nj), k = (int)(c / m.plane);
   const double* q = Qin + (long)v * m.n;
-  W[planeQ(v) * m.n + c] = q[c];
+  double* qg = W + iQG(v, c, m.n);
+  double* dd = W + iD(v, c, m.n);
+  qg[0] = q[c];
   double dr[3] = { 0, 0, 0 };
   if (Gin == nullptr || Din == nullptr) {
     const int ii[5] = { wrap(i - 2, m.ni), wrap(i - 1, m.ni), i, wrap(i + 1, m.ni), wrap(i + 2, m.ni) };
@@ -143,22 +145,22 @@ __global__ void set_state_kernel(Mesh m, const double* __restrict__ Qin, const d
   }
   if (Gin != nullptr) {
 #pragma unroll
-    for (int r = 0; r < 3; r++) W[planeG(v, r) * m.n + c] = Gin[(long)(3 * v + r) * m.n + c];
+    for (int r = 0; r < 3; r++) qg[1 + r] = Gin[(long)(3 * v + r) * m.n + c];
   } else {
 #pragma unroll
     for (int r = 0; r < 3; r++) {       // grad = J0^-T grad'
       double g;
       if (m.cart) g = dr[r] / m.h[r];
       else g = m.met[(MET_J0INV + 0 + r) * m.n + c] * dr[0] + m.met[(MET_J0INV + 3 + r) * m.n + c] * dr[1] + m.met[(MET_J0INV + 6 + r) * m.n + c] * dr[2];
-      W[planeG(v, r) * m.n + c] = g;
+      qg[1 + r] = g;
     }
   }
   if (Din != nullptr) {
 #pragma unroll
-    for (int s = 0; s < 12; s++) W[planeD(v, s) * m.n + c] = Din[(long)(12 * v + s) * m.n + c];
+    for (int s = 0; s < 12; s++) dd[s] = Din[(long)(12 * v + s) * m.n + c];
   } else {
 #pragma unroll
-    for (int s = 0; s < 12; s++) W[planeD(v, s) * m.n + c] = dr[s / 4];
+    for (int s = 0; s < 12; s++) dd[s] = dr[s / 4];
   }
 }
 
@@ -167,9 +169,11 @@ __global__ void get_state_kernel(Mesh m, const double* __restrict__ W, double* _
   const long c = (long)blockIdx.x * blockDim.x + threadIdx.x;
   if (c >= m.n) return;
   const int v = blockIdx.y;
-  if (Qo) Qo[(long)v * m.n + c] = W[planeQ(v) * m.n + c];
-  if (Go) for (int r = 0; r < 3; r++) Go[(long)(3 * v + r) * m.n + c] = W[planeG(v, r) * m.n + c];
-  if (Do) for (int s = 0; s < 12; s++) Do[(long)(12 * v + s) * m.n + c] = W[planeD(v, s) * m.n + c];
+  const double* qg = W + iQG(v, c, m.n);
+  const double* dd = W + iD(v, c, m.n);
+  if (Qo) Qo[(long)v * m.n + c] = qg[0];
+  if (Go) for (int r = 0; r < 3; r++) Go[(long)(3 * v + r) * m.n + c] = qg[1 + r];
+  if (Do) for (int s = 0; s < 12; s++) Do[(long)(12 * v + s) * m.n + c] = dd[s];
 }
 
 // time step (reading S3): dt = min over cells of cfl / sum_d (|U.n_d| + c)/h_d and of the viscous cap.
@@ -183,7 +187,7 @@ __global__ void cfl_kernel(Mesh m, const double* __restrict__ W, CflPrm p, unsig
   bool bad = false;
   const long c0 = (long)kA * m.plane, c1 = c0 + (long)cnt * m.plane;
   for (long c = c0 + (long)blockIdx.x * blockDim.x + threadIdx.x; c < c1; c += (long)gridDim.x * blockDim.x) {
-    const double rho = W[c], mx = W[m.n + c], my = W[2 * m.n + c], mz = W[3 * m.n + c], E = W[4 * m.n + c];
+    const double rho = W[iQG(0, c, m.n)], mx = W[iQG(1, c, m.n)], my = W[iQG(2, c, m.n)], mz = W[iQG(3, c, m.n)], E = W[iQG(4, c, m.n)];
     const double U[3] = { mx / rho, my / rho, mz / rho };
     const double pr = (p.gamma - 1.0) * (E - 0.5 * rho * (U[0] * U[0] + U[1] * U[1] + U[2] * U[2]));
     if (!(rho > 0.0) || !(pr > 0.0)) { bad = true; continue; }
@@ -235,11 +239,14 @@ __global__ void cfl_kernel(Mesh m, const double* __restrict__ W, CflPrm p, unsig
 // buffer W [80][n] and a contiguous buffer [80][np][plane].  PACK: W -> buf, else buf -> W.
 template <bool PACK>
 __global__ void halo_kernel(double* __restrict__ W, double* __restrict__ buf, long n, long plane, int kfirst, int np) {
-  const long per = (long)np * plane;
-  const long tot = (long)NSTATE * per;
+  // per variable the planes [kfirst, kfirst + np) are one contiguous run of 4 np plane doubles (Q, G records) and one of
+  // 12 np plane doubles (D records); the buffer holds the five Q/G runs, then the five D runs
+  const long runA = 4L * np * plane, runB = 12L * np * plane;
+  const long tot = 5 * (runA + runB);
   for (long t = (long)blockIdx.x * blockDim.x + threadIdx.x; t < tot; t += (long)gridDim.x * blockDim.x) {
-    const long f = t / per, r = t - f * per;
-    double* w = W + f * n + (long)kfirst * plane + r;
+    double* w;
+    if (t < 5 * runA) { const long v = t / runA, r = t - v * runA; w = W + iQG((int)v, (long)kfirst * plane, n) + r; }
+    else { const long u = t - 5 * runA, v = u / runB, r = u - v * runB; w = W + iD((int)v, (long)kfirst * plane, n) + r; }
     if (PACK) buf[t] = *w; else *w = buf[t];
   }
 }
@@ -274,13 +281,13 @@ __global__ void bc_halo_kernel(double* __restrict__ W, long n, long plane, int n
   double out;
   if (bc.kind <= 1) {
     const bool odd = (v == 3) || (bc.kind == 1 && (v == 1 || v == 2));
-    out = (odd ? -sgn : sgn) * W[(long)fs * n + (long)ks * plane + ij];
+    out = (odd ? -sgn : sgn) * W[iField(fs, (long)ks * plane + ij, n)];
   } else if (bc.kind == 2) {
-    out = kderiv ? 0.0 : W[(long)f * n + (long)ks * plane + ij];
+    out = kderiv ? 0.0 : W[iField(f, (long)ks * plane + ij, n)];
   } else {
     out = (f < 5) ? bc.far[f] : 0.0;
   }
-  W[(long)f * n + (long)kt * plane + ij] = out;
+  W[iField(f, (long)kt * plane + ij, n)] = out;
 }
 
 }  // namespace cgks

@@ -45,11 +45,13 @@ template <int AX> __device__ __forceinline__ void eval_axis(const double* a, dou
 
 template <bool CART>
 struct ReconCell {
-  const Mesh& m; const double* q; const double* G0; const double* G1; const double* G2;
+  const Mesh& m; const double* qg;      // records { Q, G (3) } of this variable, [n][4]
   double J[9];
-  // (grad Q)' = J0^T grad Q of neighbour cn with the TARGET cell's J0
-  __device__ __forceinline__ void grad_ref(long cn, double* gr) const {
-    const double g0 = G0[cn], g1 = G1[cn], g2 = G2[cn];
+  // average difference and (grad Q)' = J0^T grad Q of neighbour cn with the TARGET cell's J0: one 256-bit load
+  __device__ __forceinline__ void neighbour(long cn, double q0, double& dq, double* gr) const {
+    double q, g0, g1, g2;
+    ld4_ro(qg + 4 * cn, q, g0, g1, g2);
+    dq = q - q0;
     if (CART) { gr[0] = m.h[0] * g0; gr[1] = m.h[1] * g1; gr[2] = m.h[2] * g2; }
     else {
 #pragma unroll
@@ -67,8 +69,7 @@ __device__ __forceinline__ void recon_gather_axis(const ReconCell<CART>& rc, con
     op[AX] = 2; om[AX] = 0;
     const long cp = cell_at(m, ii[op[0]], jj[op[1]], kk[op[2]]), cm = cell_at(m, ii[om[0]], jj[om[1]], kk[om[2]]);
     double x[8];
-    x[0] = rc.q[cp] - q0; x[1] = rc.q[cm] - q0;
-    rc.grad_ref(cp, x + 2); rc.grad_ref(cm, x + 5);
+    rc.neighbour(cp, q0, x[0], x + 2); rc.neighbour(cm, q0, x[1], x + 5);
     dface[2 * AX] = x[0]; dface[2 * AX + 1] = x[1];
     acc_face<AX>(x, a);
   }
@@ -81,8 +82,7 @@ __device__ __forceinline__ void recon_gather_axis(const ReconCell<CART>& rc, con
       const int s1 = ((t >> 1) & 1) ? 1 : -1, s2 = (t & 1) ? 1 : -1;
       o[o1] += s1; o[o2] += s2;
       const long cn = cell_at(m, ii[o[0]], jj[o[1]], kk[o[2]]);
-      x[t] = rc.q[cn] - q0;
-      double gr[3]; rc.grad_ref(cn, gr);
+      double gr[3]; rc.neighbour(cn, q0, x[t], gr);
       x[4 + 2 * t] = gr[AX];
       x[5 + 2 * t] = s1 * gr[o1] + s2 * gr[o2];
     }
@@ -102,34 +102,32 @@ __global__ void __launch_bounds__(128, 3) recon_kernel(Mesh m, Slab sl, const do
   const CellIdx x = cell_of(m, t, kA);
   const long n = m.n;
   if (v == 0) {      // physical admissibility of the incoming cell average (reported by cgks_status / cgks_compute_dt)
-    const double rho = W[x.c], mx = W[n + x.c], my = W[2 * n + x.c], mz = W[3 * n + x.c], E = W[4 * n + x.c];
+    const double rho = W[iQG(0, x.c, n)], mx = W[iQG(1, x.c, n)], my = W[iQG(2, x.c, n)], mz = W[iQG(3, x.c, n)], E = W[iQG(4, x.c, n)];
     if (!(rho > 0.0) || !(E - 0.5 * (mx * mx + my * my + mz * mz) / rho > 0.0)) atomicOr(flag, 1);
   }
   const int ii[3] = { wrap(x.i - 1, m.ni), x.i, wrap(x.i + 1, m.ni) };
   const int jj[3] = { wrap(x.j - 1, m.nj), x.j, wrap(x.j + 1, m.nj) };
   const int kk[3] = { wrap(x.k - 1, m.nk), x.k, wrap(x.k + 1, m.nk) };
-  ReconCell<CART> rc{ m, W + (long)planeQ(v) * n, W + (long)planeG(v, 0) * n, W + (long)planeG(v, 1) * n, W + (long)planeG(v, 2) * n, {} };
+  ReconCell<CART> rc{ m, W + iQG(v, 0, n), {} };
   if (!CART) {
 #pragma unroll
     for (int q = 0; q < 9; q++) rc.J[q] = m.met[(MET_J0 + q) * n + x.c];
   }
-  const double q0 = rc.q[x.c];
+  const double q0 = rc.qg[4 * x.c];
   double a[34], dface[6], la[3];
 #pragma unroll
   for (int b = 0; b < 34; b++) a[b] = 0.0;
   recon_gather_axis<CART, 0>(rc, ii, jj, kk, q0, a, dface);
   recon_gather_axis<CART, 1>(rc, ii, jj, kk, q0, a, dface);
   recon_gather_axis<CART, 2>(rc, ii, jj, kk, q0, a, dface);
-  {   // line differences (Eq. 10): raw D, the factor h3' is folded into the coefficients
+  {   // line differences (Eq. 10): raw D, the factor h3' is folded into the coefficients; three 256-bit loads
+    const double* dd = W + iD(v, x.c, n);
     double Dl[4];
-#pragma unroll
-    for (int s = 0; s < 4; s++) Dl[s] = W[(long)planeD(v, s) * n + x.c];
+    ld4_ro(dd, Dl[0], Dl[1], Dl[2], Dl[3]);
     la[0] = 0.25 * (Dl[0] + Dl[1] + Dl[2] + Dl[3]); acc_line<0>(Dl, a);
-#pragma unroll
-    for (int s = 0; s < 4; s++) Dl[s] = W[(long)planeD(v, 4 + s) * n + x.c];
+    ld4_ro(dd + 4, Dl[0], Dl[1], Dl[2], Dl[3]);
     la[1] = 0.25 * (Dl[0] + Dl[1] + Dl[2] + Dl[3]); acc_line<1>(Dl, a);
-#pragma unroll
-    for (int s = 0; s < 4; s++) Dl[s] = W[(long)planeD(v, 8 + s) * n + x.c];
+    ld4_ro(dd + 8, Dl[0], Dl[1], Dl[2], Dl[3]);
     la[2] = 0.25 * (Dl[0] + Dl[1] + Dl[2] + Dl[3]); acc_line<2>(Dl, a);
   }
   double chi = 1.0;
@@ -226,7 +224,7 @@ __global__ void __launch_bounds__(128) diag_kernel(Mesh m, Slab sl, const double
       double pe = w[4] - 0.5 * (w[1] * w[1] + w[2] * w[2] + w[3] * w[3]) / w[0];
       if (!admissible(w)) {                    // positivity fallback (reading R9): cell average, zero gradient
 #pragma unroll
-        for (int c = 0; c < 5; c++) w[c] = W[(long)c * m.n + x.c];
+        for (int c = 0; c < 5; c++) w[c] = W[iQG(c, x.c, m.n)];
 #pragma unroll
         for (int c = 0; c < 4; c++) { g[c][0] = 0.0; g[c][1] = 0.0; g[c][2] = 0.0; }
         pe = w[4] - 0.5 * (w[1] * w[1] + w[2] * w[2] + w[3] * w[3]) / w[0];
@@ -355,7 +353,7 @@ __global__ void __launch_bounds__(FLUX_TPB, FLUX_MINB) flux_kernel(Mesh m, Slab 
   {
     if (!admissible(WLg)) {
 #pragma unroll
-      for (int c = 0; c < 5; c++) WLg[c] = W[(long)c * m.n + cL];
+      for (int c = 0; c < 5; c++) WLg[c] = W[iQG(c, cL, m.n)];
 #pragma unroll
       for (int c = 0; c < 15; c++) gL[c] = 0.0;
     }
@@ -363,7 +361,7 @@ __global__ void __launch_bounds__(FLUX_TPB, FLUX_MINB) flux_kernel(Mesh m, Slab 
       FluxPoint fp; flux_point<AXIS>(m, sl, tile, tiles_per_q, ncells, kA, fp);
       const long cr = cell_at(m, fp.ir, fp.jr, fp.kr);
 #pragma unroll
-      for (int c = 0; c < 5; c++) WRg[c] = W[(long)c * m.n + cr];
+      for (int c = 0; c < 5; c++) WRg[c] = W[iQG(c, cr, m.n)];
 #pragma unroll
       for (int c = 0; c < 15; c++) gR[c] = 0.0;
     }
@@ -499,25 +497,27 @@ __global__ void __launch_bounds__(128) update_kernel(Mesh m, Slab sl, const doub
     L *= iv;
 #pragma unroll
     for (int r = 0; r < 3; r++) SG0[r] *= iv;
-    const double qn = Wcur[(long)planeQ(v) * n + x.c];
-    Wstar[(long)planeQ(v) * n + x.c] = qn + 0.5 * dt * L + 0.125 * dt * dt * Lt;
-    Wsave[(long)planeQ(v) * n + x.c] = qn + dt * L + (1.0 / 6.0) * dt * dt * Lt;
+    const double qn = Wcur[iQG(v, x.c, n)];
+    const double hdt = 0.5 * dt;
+    st4(Wstar + iQG(v, x.c, n), qn + hdt * L + 0.125 * dt * dt * Lt, SG0[0] + hdt * SG1[0], SG0[1] + hdt * SG1[1], SG0[2] + hdt * SG1[2]);
+    st4(Wsave + iQG(v, x.c, n), qn + dt * L + (1.0 / 6.0) * dt * dt * Lt, SG0[0], SG0[1], SG0[2]);
+    double* ds = Wstar + iD(v, x.c, n); double* dv = Wsave + iD(v, x.c, n);
 #pragma unroll
-    for (int r = 0; r < 3; r++) {
-      Wstar[(long)planeG(v, r) * n + x.c] = SG0[r] + 0.5 * dt * SG1[r];
-      Wsave[(long)planeG(v, r) * n + x.c] = SG0[r];
-    }
-#pragma unroll
-    for (int s = 0; s < 12; s++) {
-      Wstar[(long)planeD(v, s) * n + x.c] = SD0[s] + 0.5 * dt * SD1[s];
-      Wsave[(long)planeD(v, s) * n + x.c] = SD0[s];
+    for (int s = 0; s < 12; s += 4) {
+      st4(ds + s, SD0[s] + hdt * SD1[s], SD0[s + 1] + hdt * SD1[s + 1], SD0[s + 2] + hdt * SD1[s + 2], SD0[s + 3] + hdt * SD1[s + 3]);
+      st4(dv + s, SD0[s], SD0[s + 1], SD0[s + 2], SD0[s + 3]);
     }
   } else {
-    Wsave[(long)planeQ(v) * n + x.c] += (1.0 / 3.0) * dt * dt * Lt;
+    double* qg = Wsave + iQG(v, x.c, n);
+    double a0, a1, a2, a3;
+    ld4(qg, a0, a1, a2, a3);
+    st4(qg, a0 + (1.0 / 3.0) * dt * dt * Lt, a1 + dt * SG1[0], a2 + dt * SG1[1], a3 + dt * SG1[2]);
+    double* dv = Wsave + iD(v, x.c, n);
 #pragma unroll
-    for (int r = 0; r < 3; r++) Wsave[(long)planeG(v, r) * n + x.c] += dt * SG1[r];
-#pragma unroll
-    for (int s = 0; s < 12; s++) Wsave[(long)planeD(v, s) * n + x.c] += dt * SD1[s];
+    for (int s = 0; s < 12; s += 4) {
+      ld4(dv + s, a0, a1, a2, a3);
+      st4(dv + s, a0 + dt * SD1[s], a1 + dt * SD1[s + 1], a2 + dt * SD1[s + 2], a3 + dt * SD1[s + 3]);
+    }
   }
 }
 
