@@ -148,8 +148,21 @@ def build_matrices():
     return M, E, Gram, A
 
 
+CANON = []      # canonical values of the emitted constants
+
+
 def lit(v):
-    return repr(float(v))
+    """A coefficient as a literal.  Coefficients that are mathematically equal come out of the numerical null-space / quadrature
+    construction with different last bits; they are snapped to one representative (relative distance <= 1e-13), so that
+    ptxas can share the two UMOV instructions that materialise an FP64 literal among the FMAs that use it."""
+    v = float(v)
+    for c in CANON:
+        if abs(v - c) <= 1e-13 * abs(c):
+            return repr(c)
+        if abs(v + c) <= 1e-13 * abs(c):
+            return repr(-c)
+    CANON.append(v)
+    return repr(v)
 
 
 # ------------------------------------------------------------------------------------------------------------------
@@ -373,6 +386,7 @@ def emit_quadform(name, Gm):
 
 
 def generate(path):
+    del CANON[:]
     M, E, Gram, A = build_matrices()
     B = basis_indices()
     combos, nnzS = parity_combos(A, B, M)
