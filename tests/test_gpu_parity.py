@@ -1,6 +1,8 @@
 """GPU parity tests: the CUDA path (through the C ABI) against the CPU oracle, element by element, on the same
 seeded inputs.  Tolerances (BASELINE.json north_star): relative L-inf <= 1e-10 after one step and <= 1e-8 after
 100 steps, on every one of the 80 fields (norm of DESIGN.md section 6)."""
+import os
+
 import numpy as np
 import pytest
 
@@ -482,7 +484,7 @@ def _block_nodes(nodes, lo, B):
 
 
 @pytest.mark.parametrize("case", ["iso_sup_384_after_100", "iso_sub_128_after_100", "tgv_sup_128_shocked", "tgv_curv_64_after_100",
-                                  "iso_sup_64_rough_after_50"])
+                                  "iso_sup_64_rough_after_50", "tgv_sup_320_shocked"])
 def test_restart_parity(case):
     """Multi-step and shock-active states at sizes the oracle cannot run as a whole (north_star: 100 steps on all five
     configs; Ma = 1.25 vortex once shocklets have formed): the library runs the steps on the full
@@ -507,10 +509,15 @@ def test_restart_parity(case):
         nodes = inputs.cartesian_nodes(n)
         Q = inputs.iso_turbulence(n, 4, 0.5, 8.0, device=dev).contiguous()
         budget = 0
-    elif case == "tgv_sup_128_shocked":
-        n, steps, B, nb = 128, 0, 24, 6
+    elif case in ("tgv_sup_128_shocked", "tgv_sup_320_shocked"):
+        n = 128 if "128" in case else 320               # the two mesh sizes of the paper's Ma = 1.25 runs
+        if n == 320 and not os.environ.get("CGKS_LONG_TESTS"):
+            pytest.skip("about 1400 steps at 320^3 (5 GPU-minutes): set CGKS_LONG_TESTS=1; result recorded in DESIGN.md 9b")
+        if n == 320 and free < 150e9:
+            pytest.skip("needs a 180 GB device")
+        steps, B, nb = 0, 24, 6
         w = inputs.workload("tgv_sup", n); prm = w["params"]; nonlinear = 1; nodes = w["nodes"]; Q = w["Q"]
-        budget = 0
+        budget = 0 if n == 128 else int(free - 30e9)
     elif case == "tgv_curv_64_after_100":
         n, steps, B, nb = 64, 100, 24, 4
         w = inputs.workload("tgv_curv", n); prm = w["params"]; nonlinear = 1; nodes = w["nodes"]; Q = w["Q"]
@@ -524,7 +531,7 @@ def test_restart_parity(case):
     s = binding.Solver(nodes, binding.make_params(**prm, nonlinear=nonlinear), device=dev, budget_bytes=budget)
     s.set_state(Q)
     del Q
-    if case == "tgv_sup_128_shocked":
+    if case.startswith("tgv_sup"):
         t = 0.0
         while t < 3.5:                      # shocklets of the Ma = 1.25 vortex form from t ~ 3
             dt = s.compute_dt(0.5); s.step(dt); t += dt
@@ -533,7 +540,7 @@ def test_restart_parity(case):
             s.step(s.compute_dt(0.5))
     s.status()
     lows = [tuple(int(v) for v in rng.integers(0, n, 3)) for _ in range(nb)]
-    if case == "tgv_sup_128_shocked":
+    if case.startswith("tgv_sup"):
         # blocks around the cells where the adaptive weights respond most (smallest chi of the density)
         s.step(s.compute_dt(0.5)); chi = s.chi()[0]
         flat = torch.argsort(chi.flatten())[:: max(1, chi.numel() // 400000)][:3].cpu().numpy()
