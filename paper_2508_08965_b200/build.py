@@ -7,7 +7,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libcgks.so")
 SOURCES = ["cgks_api.cu"]
-HEADERS = ["cgks_common.cuh", "kernels_setup.cuh", "kernels_stage.cuh", "gks_flux.cuh", "fastmath64.cuh", "recon_gen.cuh", "math_gen.cuh"]
+HEADERS = ["cgks_common.cuh", "kernels_setup.cuh", "kernels_stage.cuh", "kernels_fused.cuh", "gks_flux.cuh", "fastmath64.cuh", "recon_gen.cuh", "math_gen.cuh"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared"]
 

@@ -3,9 +3,11 @@
 #include "cgks_common.cuh"
 #include "kernels_setup.cuh"
 #include "kernels_stage.cuh"
+#include "kernels_fused.cuh"
 
 #include <math.h>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 #include <string>
 #include <vector>
@@ -23,7 +25,8 @@ struct EvRec { int cls; cudaEvent_t a, b; };
 
 size_t align_up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
 size_t state_bytes(long n) { return align_up((size_t)NSTATE * n * 8); }
-size_t slot_bytes(long plane) { return (size_t)(NPV + NFX) * plane * 8; }
+size_t slot_bytes(long plane) { return (size_t)(NPV + NFX) * plane * 8; }      // three-kernel pipeline: pv + fx
+size_t slot_bytes_pv(long plane) { return (size_t)NPV * plane * 8; }           // sweep pipeline: pv only
 }  // namespace
 
 struct cgks_ctx {
@@ -43,6 +46,8 @@ struct cgks_ctx {
   int kofs = 0, nk_global = 0;          // global plane of local plane 0 (may be negative: wraps), planes of the global mesh
   int phase = 0;                        // sub-domain: 0 = next is stage 1 (input W[cur]), 1 = next is stage 2 (input W[star])
   int S = 0;                            // slab depth in k-planes; S == nk: whole mesh resident
+  int sweep_minseg = 24;                // shortest segment of a j / k line of the sweep kernels
+  int split = 0;                        // 1: three-kernel pipeline (flux -> fx -> update) instead of the sweep kernels
   int slots_pv = 0, slots_fx = 0;
   long launches = 0;
   int profiling = 0;
@@ -132,6 +137,12 @@ static cudaError_t set_flux_smem() {
   CGKS_ATTR(false, 0, true); CGKS_ATTR(false, 1, true); CGKS_ATTR(false, 2, true);
   CGKS_ATTR(false, 0, false); CGKS_ATTR(false, 1, false); CGKS_ATTR(false, 2, false);
 #undef CGKS_ATTR
+#define CGKS_ATTR(C, A, ST) if (e == cudaSuccess) e = cudaFuncSetAttribute(sweep_kernel<C, A, ST>, cudaFuncAttributeMaxDynamicSharedMemorySize, SW_SMEM_BYTES)
+  CGKS_ATTR(true, 0, 1); CGKS_ATTR(true, 1, 1); CGKS_ATTR(true, 2, 1);
+  CGKS_ATTR(true, 0, 2); CGKS_ATTR(true, 1, 2); CGKS_ATTR(true, 2, 2);
+  CGKS_ATTR(false, 0, 1); CGKS_ATTR(false, 1, 1); CGKS_ATTR(false, 2, 1);
+  CGKS_ATTR(false, 0, 2); CGKS_ATTR(false, 1, 2); CGKS_ATTR(false, 2, 2);
+#undef CGKS_ATTR
   return e;
 }
 
@@ -152,6 +163,7 @@ static int create_impl(cgks_ctx** out, int ni, int nj, int nkg, int nk, int kofs
   cgks_ctx* c = new cgks_ctx();
   c->prm = *params; c->stream = (cudaStream_t)stream;
   c->open_k = open_k; c->kofs = kofs; c->nk_global = nkg;
+  { const char* e = getenv("CGKS_PIPELINE"); c->split = (e && strcmp(e, "split") == 0) ? 1 : 0; }
   {
     int dev = 0; cudaGetDevice(&dev);
     if (cudaDeviceGetAttribute(&c->nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || c->nsm <= 0) c->nsm = 148;
@@ -201,9 +213,11 @@ static int create_impl(cgks_ctx** out, int ni, int nj, int nkg, int nk, int kofs
       e = cudaStreamSynchronize(c->stream);
       if (e != cudaSuccess) { c->err = std::string("geometry pass 2: ") + cudaGetErrorString(e); rc = CGKS_ECUDA; break; }
     }
-    // slab buffers from what is left
+    // slab buffers from what is left.  Sweep pipeline (default): reconstructed face values (pv) only; the face-flux buffer
+    // (fx) exists only when the whole mesh is resident and there is room (test tap cgks_debug_stage) or in the three-kernel
+    // pipeline (CGKS_PIPELINE=split, kept for A/B timing).
     const size_t left = (size_t)(end - p);
-    const size_t sb = slot_bytes(m.plane);
+    const size_t sb = c->split ? slot_bytes(m.plane) : slot_bytes_pv(m.plane);
     long slots = (long)(left / sb);
     if (slots >= nk) { c->S = nk; c->slots_pv = nk; c->slots_fx = nk; }
     else {
@@ -214,7 +228,7 @@ static int create_impl(cgks_ctx** out, int ni, int nj, int nkg, int nk, int kofs
       c->S = (int)S; c->slots_pv = (int)S + 2; c->slots_fx = (int)S + 1;
     }
     c->pv = (double*)p; p += (size_t)NPV * c->slots_pv * m.plane * 8;
-    c->fx = (double*)p;
+    c->fx = (c->split || (size_t)(end - p) >= (size_t)NFX * c->slots_fx * m.plane * 8) ? (double*)p : nullptr;
     cudaMemsetAsync(c->d_flags, 0, 64, c->stream);
   } while (0);
   if (rc != CGKS_OK) { g_create_err = c->err; delete c; return rc; }      // message: cgks_last_create_error()
@@ -317,6 +331,39 @@ static void launch_flux(cgks_ctx* c, const Slab& sl, const double* Win, double d
 #undef CGKS_FLUX
 }
 
+static int wrapk(int k, int nk) { return k < 0 ? k + nk : (k >= nk ? k - nk : k); }
+
+// the sweep pipeline: per direction ONE kernel does flux + update of planes kA .. kA+cnt-1 (kernels_fused.cuh)
+template <bool CART>
+static void launch_sweeps(cgks_ctx* c, const Slab& sl, const double* Win, double dt, int kA, int cnt, int stage) {
+  const Mesh& m = c->mesh;
+  const GasConst gc = gas_const(c->prm);
+  const double idt = 1.0 / dt;
+  const long maxb = (long)c->nsm * FLUX_MINB;
+  SweepPrm sp; sp.kA = kA; sp.cnt = cnt; sp.ntx = (m.ni + SW_CELLS - 1) / SW_CELLS;
+  double* Wcur = c->W[c->cur]; double* Wstar = c->W[c->star]; double* Wsave = c->W[c->save];
+  auto lines = [&](int ax) {
+    // lines along j / k are cut into segments so that every warp gets many lines (each segment recomputes one face)
+    const int len = ax == 1 ? m.nj : cnt;
+    sp.seg = len; sp.nseg = 1;
+    if (ax != 0) {
+      const long want = 32L * maxb * (SW_TPB / 32);
+      const long full = (long)sp.ntx * (ax == 1 ? cnt : m.nj);
+      long nseg = (want + full - 1) / full; if (nseg < 1) nseg = 1;
+      long seg = (len + nseg - 1) / nseg; if (seg < c->sweep_minseg) seg = c->sweep_minseg; if (seg > len) seg = len;
+      sp.seg = (int)seg; sp.nseg = (int)((len + seg - 1) / seg);
+    }
+    sp.nlines = ax == 0 ? cnt * m.nj : (ax == 1 ? cnt * sp.nseg * sp.ntx : sp.nseg * m.nj * sp.ntx);
+    const long nb = ((long)sp.nlines + SW_TPB / 32 - 1) / (SW_TPB / 32);
+    return (unsigned)(nb < maxb ? nb : maxb);
+  };
+#define CGKS_SWEEP(AX) do { const unsigned grid = lines(AX); Timed t(c, KC_FLUX); \
+    if (stage == 2) sweep_kernel<CART, AX, 2><<<grid, SW_TPB, SW_SMEM_BYTES, c->stream>>>(m, sl, sp, Win, c->pv, Wcur, Wstar, Wsave, gc, dt, idt); \
+    else sweep_kernel<CART, AX, 1><<<grid, SW_TPB, SW_SMEM_BYTES, c->stream>>>(m, sl, sp, Win, c->pv, Wcur, Wstar, Wsave, gc, dt, idt); } while (0)
+  CGKS_SWEEP(0); CGKS_SWEEP(1); CGKS_SWEEP(2);
+#undef CGKS_SWEEP
+}
+
 template <bool CART>
 static void run_stage(cgks_ctx* c, int stage, double dt) {
   const Mesh& m = c->mesh;
@@ -337,12 +384,18 @@ static void run_stage(cgks_ctx* c, int stage, double dt) {
     if (stage == 1) update_kernel<CART, 1><<<grid, TPB, 0, c->stream>>>(m, sl, c->fx, c->W[c->cur], c->W[c->star], c->W[c->save], dt, kA, nt);
     else update_kernel<CART, 2><<<grid, TPB, 0, c->stream>>>(m, sl, c->fx, c->W[c->cur], c->W[c->star], c->W[c->save], dt, kA, nt);
   };
+  // flux + update of planes kA .. kA+cnt-1: three sweep kernels (i, j, k), or flux x 3 -> fx -> update
+  auto advance = [&](int kA, int cnt) {
+    if (c->split) { launch_flux<CART>(c, sl, Win, dt, wrapk(kA - 1, m.nk), cnt + 1, stage); update(kA, cnt); }
+    else launch_sweeps<CART>(c, sl, Win, dt, kA, cnt, stage);
+  };
   if (c->S >= m.nk) {                       // whole mesh resident: no recomputation
     sl.kbase = 0;
     if (c->open_k) {                        // sub-domain: planes 0, 1 and nk-2, nk-1 are halos (filled by cgks_unpack_halo)
-      recon(1, m.nk - 2); launch_flux<CART>(c, sl, Win, dt, 1, m.nk - 3, stage); update(2, m.nk - 4);
+      recon(1, m.nk - 2); advance(2, m.nk - 4);
     } else {
-      recon(0, m.nk); launch_flux<CART>(c, sl, Win, dt, 0, m.nk, stage); update(0, m.nk);
+      recon(0, m.nk);
+      if (c->split) { launch_flux<CART>(c, sl, Win, dt, 0, m.nk, stage); update(0, m.nk); } else advance(0, m.nk);
     }
     return;
   }
@@ -351,8 +404,7 @@ static void run_stage(cgks_ctx* c, int stage, double dt) {
     const int k1 = (k0 + c->S < kend) ? k0 + c->S : kend;
     sl.kbase = (k0 == 0) ? m.nk - 1 : k0 - 1;
     recon(sl.kbase, k1 - k0 + 2);                                   // planes k0-1 .. k1
-    launch_flux<CART>(c, sl, Win, dt, sl.kbase, k1 - k0 + 1, stage); // cells of planes k0-1 .. k1-1 own the needed faces
-    update(k0, k1 - k0);
+    advance(k0, k1 - k0);                                           // faces of planes k0-1 .. k1-1, cells of planes k0 .. k1-1
   }
 }
 
@@ -431,6 +483,7 @@ extern "C" int cgks_debug_stage(cgks_ctx* c, double dt, double* d_pv, double* d_
   else recon_kernel<false><<<grid, TPB, 0, c->stream>>>(m, sl, Win, c->pv, c->chi, rp, 0, nt, c->d_flags + 3);
   c->launches++;
   if (d_pv) { pv_unpack_kernel<<<dim3((unsigned)((nt + TPB - 1) / TPB), 24 * NVAR), TPB, 0, c->stream>>>(sl, m.n, c->pv, d_pv); c->launches++; }
+  if (d_fx && !c->fx) return fail(c, CGKS_ENOMEM, "flux tap: the workspace has no room for the face-flux buffer");
   if (d_fx) {
     if (m.cart) launch_flux<true>(c, sl, Win, dt, 0, m.nk, 1); else launch_flux<false>(c, sl, Win, dt, 0, m.nk, 1);
     CK(cudaMemcpyAsync(d_fx, c->fx, (size_t)NFX * m.n * 8, cudaMemcpyDeviceToDevice, c->stream));
@@ -449,14 +502,15 @@ static void run_diagnostics(cgks_ctx* c, double* d_acc) {
   Slab sl; sl.slots_pv = c->slots_pv; sl.slots_fx = c->slots_fx;
   sl.stride_pv = (long)c->slots_pv * m.plane; sl.stride_fx = (long)c->slots_fx * m.plane;
   const int S = c->S >= m.nk ? m.nk : c->S;
+  double* scratch = c->pv + 4 * (long)(8 * NVAR) * sl.stride_pv;      // per-block partials: behind the 8 x 5 record planes the volume points use
   for (int k0 = 0; k0 < m.nk; k0 += S) {
     const int cnt = (k0 + S < m.nk) ? S : m.nk - k0;
     sl.kbase = k0;
     const long nt = (long)cnt * m.plane;
     const unsigned nb = (unsigned)((nt + TPB - 1) / TPB);
     { Timed t(c, KC_OTHER); recon_kernel<CART, true><<<dim3(nb, 5), TPB, 0, c->stream>>>(m, sl, Win, c->pv, nullptr, rp, k0, nt, c->d_flags + 3); }
-    { Timed t(c, KC_OTHER); diag_kernel<CART><<<nb, TPB, 0, c->stream>>>(m, sl, Win, c->pv, dp, k0, nt, c->fx); }     // fx = scratch for the partials
-    { Timed t(c, KC_OTHER); diag_reduce_kernel<<<1, 256, 0, c->stream>>>(c->fx, (long)nb, d_acc); }
+    { Timed t(c, KC_OTHER); diag_kernel<CART><<<nb, TPB, 0, c->stream>>>(m, sl, Win, c->pv, dp, k0, nt, scratch); }
+    { Timed t(c, KC_OTHER); diag_reduce_kernel<<<1, 256, 0, c->stream>>>(scratch, (long)nb, d_acc); }
   }
 }
 

@@ -1,0 +1,345 @@
+// kernels_fused.cuh -- the gas-kinetic flux (row a4) and the update / S2O4 combine (row a5) of a stage as ONE sweep kernel per
+// face direction: the interface results never go to HBM (the fx buffer of the three-kernel split, 2880 / 1440 B per cell
+// and stage written and read back, is gone, and with it the update kernel).
+//
+//   sweep_kernel<CART, AXIS, STAGE>   PAPER.md:33-92, 330-352 (Eq. 1-7) at the Gauss points of the + faces of direction AXIS,
+//                                     then Eq. 8-10 restricted to the two faces of that direction and the
+//                                     S2O4 combine, accumulated into the state buffers direction by direction.
+//
+// Mapping.  A WARP owns a tile of 8 cells along i x the 4 Gauss points of their + face of direction AXIS (lane = 4 cell + q)
+// and marches along a line of such tiles in the direction AXIS, one tile per step.  The face computed in the previous step
+// is the - face of the cells of this step: what it hands over (F^n, F_t^n and the right-hand interface values, 20 numbers
+// per point) stays in shared memory -- for AXIS = 1, 2 in the thread's own slot, for AXIS = 0 in the slot of the lane four to
+// the right (the first cell of a tile takes the last cell of the previous tile).  Every line starts with one extra step (the
+// face below its first cell: for AXIS = 0 the periodic image of the row's last face, computed by four lanes).
+// The sums over the four Gauss points of a face (Eq. 8-9) are two butterfly shuffles inside the quad; lane q then owns
+// component q of the cell's record { Q, G_x, G_y, G_z } and line difference 4 AXIS + q of the 12 (Eq. 10): a quad reads and
+// writes whole 32-byte sectors.  Direction 0 of stage 1 writes the records, the later directions (and every direction of stage
+// 2, which updates the saved buffer in place) read-modify-write them; these operands are prefetched with cp.async together
+// with the 2 x 20 reconstructed inputs of the next step, one step ahead of the arithmetic.  No block-level synchronisation,
+// no atomics: the order of every floating-point sum is fixed, results are deterministic and independent of the slab depth.
+#pragma once
+#include "kernels_stage.cuh"
+
+namespace cgks {
+
+constexpr int SW_TPB = 128;                  // 4 warps; FLUX_MINB blocks per SM (254 registers per thread)
+constexpr int SW_CELLS = 8;                  // cells per warp tile
+constexpr int SW_SMEM_IN = 40 * SW_TPB;      // doubles: staged inputs [20 chunks][SW_TPB][2]
+constexpr int SW_SMEM_X = 20 * SW_TPB;       // doubles: hand-over values [20][SW_TPB]
+constexpr int SW_SMEM_RMW = 2 * 10 * SW_TPB; // doubles: read-modify-write operands [2 (step parity)][10][SW_TPB]
+constexpr int SW_SMEM_BYTES = (SW_SMEM_IN + SW_SMEM_X + SW_SMEM_RMW) * 8;
+
+struct SweepPrm {
+  int kA, cnt;       // planes kA .. kA+cnt-1 (wrapped) are updated
+  int seg, nseg;     // lines along AXIS = 1 (j) or 2 (k) are cut into nseg segments of seg cells
+  int ntx;           // tiles per row: ceil(ni / 8)
+  int nlines;
+};
+
+__device__ __forceinline__ void cp_async8(double* smem_dst, const double* gsrc) {
+  const unsigned sa = (unsigned)__cvta_generic_to_shared(smem_dst);
+  const size_t ga = __cvta_generic_to_global(gsrc);
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(sa), "l"(ga) : "memory");
+}
+
+// a line and this lane's cell at its step 0
+struct SweepLine { int len, i, j, k; };
+
+template <int AXIS>
+__device__ __forceinline__ SweepLine sweep_line(const Mesh& m, const SweepPrm& sp, int line, int cl) {
+  SweepLine L;
+  const unsigned u = (unsigned)line;
+  if (AXIS == 0) {
+    const unsigned kk = u / (unsigned)m.nj;
+    L.j = (int)(u - kk * (unsigned)m.nj); L.k = sp.kA + (int)kk; L.i = cl; L.len = sp.ntx;
+  } else if (AXIS == 1) {
+    const unsigned a = u / (unsigned)sp.ntx, tx = u - a * (unsigned)sp.ntx;
+    const unsigned kk = a / (unsigned)sp.nseg, sg = a - kk * (unsigned)sp.nseg;
+    L.i = (int)tx * SW_CELLS + cl; L.j = (int)sg * sp.seg; L.k = sp.kA + (int)kk;
+    L.len = m.nj - L.j < sp.seg ? m.nj - L.j : sp.seg;
+  } else {
+    const unsigned a = u / (unsigned)sp.ntx, tx = u - a * (unsigned)sp.ntx;
+    const unsigned sg = a / (unsigned)m.nj, j = a - sg * (unsigned)m.nj;
+    const int kk0 = (int)sg * sp.seg;
+    L.i = (int)tx * SW_CELLS + cl; L.j = (int)j; L.k = sp.kA + kk0;
+    L.len = sp.cnt - kk0 < sp.seg ? sp.cnt - kk0 : sp.seg;
+  }
+  if (L.k >= m.nk) L.k -= m.nk;
+  return L;
+}
+
+// this lane's left cell (cL), the cell across the + face (cR) and their slab offsets at step s (-1: the line's extra first face)
+struct SweepPos { bool act; int cL, cR; long offL, offR; };
+
+template <int AXIS>
+__device__ __forceinline__ SweepPos sweep_pos(const Mesh& m, const Slab& sl, const SweepLine& L, int s, int cl) {
+  SweepPos p;
+  int i = L.i, j = L.j, k = L.k;
+  if (AXIS == 0) {
+    if (s < 0) { i = m.ni - 1; p.act = (cl == SW_CELLS - 1); }
+    else { i = L.i + SW_CELLS * s; p.act = i < m.ni; }
+  } else {
+    p.act = i < m.ni;
+    if (AXIS == 1) j = wrap(j + s, m.nj); else k = wrap(k + s, m.nk);
+  }
+  int ir = i, jr = j, kr = k;
+  if (AXIS == 0) ir = wrap(i + 1, m.ni); else if (AXIS == 1) jr = wrap(j + 1, m.nj); else kr = wrap(k + 1, m.nk);
+  const int ijL = j * m.ni + i, ijR = jr * m.ni + ir;
+  p.cL = k * (int)m.plane + ijL; p.cR = kr * (int)m.plane + ijR;
+  p.offL = (long)slot_of(m, sl, k) * m.plane + ijL;
+  p.offR = (long)slot_of(m, sl, kr) * m.plane + ijR;
+  return p;
+}
+
+template <bool CART, int AXIS, int STAGE>
+__global__ void __launch_bounds__(SW_TPB, FLUX_MINB) sweep_kernel(Mesh m, Slab sl, SweepPrm sp, const double* __restrict__ Win,
+                                                                  const double* __restrict__ pv, const double* Wcur, double* Wstar,
+                                                                  double* Wsave, GasConst gc, double dt, double idt) {
+  constexpr bool STAGE2 = (STAGE == 2);
+  constexpr bool FIRST = (STAGE == 1 && AXIS == 0);      // writes the records instead of accumulating into them
+  constexpr int NX = STAGE2 ? 10 : 20;                   // numbers handed to the next cell per point
+  extern __shared__ __align__(16) double sm[];
+  double* smf = sm;                                      // staged inputs
+  double* smx = sm + SW_SMEM_IN;                         // hand-over values
+  double* smr = sm + SW_SMEM_IN + SW_SMEM_X;             // read-modify-write operands
+  const int tid = threadIdx.x, lane = tid & 31, q = lane & 3, cl = lane >> 2;
+  const int gw = blockIdx.x * (SW_TPB / 32) + (tid >> 5), nw = gridDim.x * (SW_TPB / 32);
+  const long n = m.n;
+
+  // ---- staging of one step's inputs: 2 x 5 records of the reconstruction + the operands of the read-modify-write
+  auto issue = [&](const SweepPos& p, int s, int par) {
+    if (p.act) {
+      const double* pL = pv + pv_index(sl, 4 * (2 * AXIS) + q, 0, p.offL);
+      const double* pR = pv + pv_index(sl, 4 * (2 * AXIS + 1) + q, 0, p.offR);
+      double* dst = smf + 2 * tid;
+#pragma unroll
+      for (int c = 0; c < 10; c++) cp_async16(dst + c * (2 * SW_TPB), pL + (long)(c >> 1) * (4 * sl.stride_pv) + 2 * (c & 1));
+#pragma unroll
+      for (int c = 0; c < 10; c++) cp_async16(dst + (10 + c) * (2 * SW_TPB), pR + (long)(c >> 1) * (4 * sl.stride_pv) + 2 * (c & 1));
+      if (s >= 0) {
+        double* r = smr + par * (10 * SW_TPB) + tid;
+        if (FIRST) {
+          if (q == 0) {
+#pragma unroll
+            for (int v = 0; v < 5; v++) cp_async8(r + v * SW_TPB, Wcur + iQG(v, p.cL, n));
+          }
+        } else if (!STAGE2) {
+#pragma unroll
+          for (int v = 0; v < 5; v++) { cp_async8(r + v * SW_TPB, Wstar + iQG(v, p.cL, n) + q); cp_async8(r + (5 + v) * SW_TPB, Wsave + iQG(v, p.cL, n) + q); }
+        } else {
+#pragma unroll
+          for (int v = 0; v < 5; v++) { cp_async8(r + v * SW_TPB, Wsave + iQG(v, p.cL, n) + q); cp_async8(r + (5 + v) * SW_TPB, Wsave + iD(v, p.cL, n) + 4 * AXIS + q); }
+        }
+      }
+    }
+    cp_async_commit();
+  };
+
+  int line = gw, s = -1, par = 0;
+  if (line >= sp.nlines) return;
+  SweepLine L = sweep_line<AXIS>(m, sp, line, cl);
+  SweepPos cur = sweep_pos<AXIS>(m, sl, L, s, cl);
+  issue(cur, s, par);
+#pragma unroll 1
+  while (line < sp.nlines) {
+    cp_async_wait<0>();
+    const double2* sL = reinterpret_cast<const double2*>(smf) + tid;
+    double WLg[5], WRg[5], gL[15], gR[15];
+#pragma unroll
+    for (int v = 0; v < 5; v++) {
+      const double2 l0 = sL[(2 * v) * SW_TPB], l1 = sL[(2 * v + 1) * SW_TPB];
+      const double2 r0 = sL[(10 + 2 * v) * SW_TPB], r1 = sL[(11 + 2 * v) * SW_TPB];
+      WLg[v] = l0.x; gL[3 * v] = l0.y; gL[3 * v + 1] = l1.x; gL[3 * v + 2] = l1.y;
+      WRg[v] = r0.x; gR[3 * v] = r0.y; gR[3 * v + 1] = r1.x; gR[3 * v + 2] = r1.y;
+    }
+    // the step after this one (warp-uniform), its inputs stream in during the arithmetic of this one
+    int nline = line, ns = s + 1;
+    if (ns >= L.len) { nline = line + nw; ns = -1; if (nline < sp.nlines) L = sweep_line<AXIS>(m, sp, nline, cl); }
+    SweepPos nxt; nxt.act = false; nxt.cL = 0; nxt.cR = 0; nxt.offL = 0; nxt.offR = 0;
+    if (nline < sp.nlines) nxt = sweep_pos<AXIS>(m, sl, L, ns, cl);
+    issue(nxt, ns, par ^ 1);
+
+    const bool act = cur.act;
+    const unsigned amask = __ballot_sync(0xffffffffu, act);
+    double P[4][5];       // this face, global frame: F^n, F_t^n, own-side (left) value and time derivative
+    double R[2][5];       // right-hand interface value and time derivative: they belong to the next cell
+    double fr[3][3];
+    if (act) {
+      // positivity (reading R9, point-wise): a non-physical reconstructed state falls back to the cell average
+      if (!admissible(WLg)) {
+#pragma unroll
+        for (int c = 0; c < 5; c++) WLg[c] = Win[iQG(c, cur.cL, n)];
+#pragma unroll
+        for (int c = 0; c < 15; c++) gL[c] = 0.0;
+      }
+      if (!admissible(WRg)) {
+#pragma unroll
+        for (int c = 0; c < 5; c++) WRg[c] = Win[iQG(c, cur.cR, n)];
+#pragma unroll
+        for (int c = 0; c < 15; c++) gR[c] = 0.0;
+      }
+      double WL[5], WR[5], SL[3][5], SR[3][5];
+      if (CART) {
+        const int p0 = AXIS, p1 = (AXIS + 1) % 3, p2 = (AXIS + 2) % 3;
+        const int pm[3] = { p0, p1, p2 };
+        WL[0] = WLg[0]; WL[4] = WLg[4]; WR[0] = WRg[0]; WR[4] = WRg[4];
+#pragma unroll
+        for (int a = 0; a < 3; a++) { WL[1 + a] = WLg[1 + pm[a]]; WR[1 + a] = WRg[1 + pm[a]]; }
+#pragma unroll
+        for (int dd = 0; dd < 3; dd++) {
+          SL[dd][0] = gL[pm[dd]]; SL[dd][4] = gL[12 + pm[dd]]; SR[dd][0] = gR[pm[dd]]; SR[dd][4] = gR[12 + pm[dd]];
+#pragma unroll
+          for (int a = 0; a < 3; a++) { SL[dd][1 + a] = gL[3 * (1 + pm[a]) + pm[dd]]; SR[dd][1 + a] = gR[3 * (1 + pm[a]) + pm[dd]]; }
+        }
+      } else {
+        double A[3];
+#pragma unroll
+        for (int r = 0; r < 3; r++) { A[r] = m.met[(MET_AREA + 3 * AXIS + r) * n + cur.cL]; fr[1][r] = m.met[(MET_TAN + 3 * AXIS + r) * n + cur.cL]; }
+        const double S = sqrt(A[0] * A[0] + A[1] * A[1] + A[2] * A[2]);
+#pragma unroll
+        for (int r = 0; r < 3; r++) fr[0][r] = A[r] / S;
+        fr[2][0] = fr[0][1] * fr[1][2] - fr[0][2] * fr[1][1];
+        fr[2][1] = fr[0][2] * fr[1][0] - fr[0][0] * fr[1][2];
+        fr[2][2] = fr[0][0] * fr[1][1] - fr[0][1] * fr[1][0];
+#pragma unroll
+        for (int side = 0; side < 2; side++) {
+          const double* Wg = side ? WRg : WLg; const double* gg = side ? gR : gL;
+          double* Wl = side ? WR : WL; double (*Sx)[5] = side ? SR : SL;
+          Wl[0] = Wg[0]; Wl[4] = Wg[4];
+#pragma unroll
+          for (int a = 0; a < 3; a++) Wl[1 + a] = Wg[1] * fr[a][0] + Wg[2] * fr[a][1] + Wg[3] * fr[a][2];
+#pragma unroll
+          for (int dd = 0; dd < 3; dd++) {
+            double dg[5];
+#pragma unroll
+            for (int vv = 0; vv < 5; vv++) dg[vv] = gg[3 * vv] * fr[dd][0] + gg[3 * vv + 1] * fr[dd][1] + gg[3 * vv + 2] * fr[dd][2];
+            Sx[dd][0] = dg[0]; Sx[dd][4] = dg[4];
+#pragma unroll
+            for (int a = 0; a < 3; a++) Sx[dd][1 + a] = dg[1] * fr[a][0] + dg[2] * fr[a][1] + dg[3] * fr[a][2];
+          }
+        }
+      }
+      double out[6][5];      // Fn, Ft, VL, DL, VR, DR in the face frame
+      gks_flux_local<STAGE2>(gc, dt, idt, WL, SL, WR, SR, out[0], out[1], out[2], out[3], out[4], out[5]);
+      // back to the global frame
+#pragma unroll
+      for (int g = 0; g < 6; g++) {
+        if (STAGE2 && (g == 0 || g == 2 || g == 4)) continue;
+        double o3[3];
+        if (CART) {
+          const int p0 = AXIS, p1 = (AXIS + 1) % 3, p2 = (AXIS + 2) % 3;
+          o3[p0] = out[g][1]; o3[p1] = out[g][2]; o3[p2] = out[g][3];
+        } else {
+#pragma unroll
+          for (int r = 0; r < 3; r++) o3[r] = out[g][1] * fr[0][r] + out[g][2] * fr[1][r] + out[g][3] * fr[2][r];
+        }
+        double* d = (g < 4) ? P[g] : R[g - 4];
+        d[0] = out[g][0]; d[1] = o3[0]; d[2] = o3[1]; d[3] = o3[2]; d[4] = out[g][4];
+      }
+    }
+    // ---- hand-over: M = what the face below this cell left (F^n, F_t^n, right-hand value and time derivative)
+    double M[4][5];
+    {
+      double* xs = smx + tid;
+      auto put = [&]() {
+        if (!STAGE2) {
+#pragma unroll
+          for (int v = 0; v < 5; v++) { xs[v * SW_TPB] = P[0][v]; xs[(5 + v) * SW_TPB] = P[1][v]; xs[(10 + v) * SW_TPB] = R[0][v]; xs[(15 + v) * SW_TPB] = R[1][v]; }
+        } else {
+#pragma unroll
+          for (int v = 0; v < 5; v++) { xs[v * SW_TPB] = P[1][v]; xs[(5 + v) * SW_TPB] = R[1][v]; }
+        }
+      };
+      auto get = [&](const double* src) {
+        if (!STAGE2) {
+#pragma unroll
+          for (int v = 0; v < 5; v++) { M[0][v] = src[v * SW_TPB]; M[1][v] = src[(5 + v) * SW_TPB]; M[2][v] = src[(10 + v) * SW_TPB]; M[3][v] = src[(15 + v) * SW_TPB]; }
+        } else {
+#pragma unroll
+          for (int v = 0; v < 5; v++) { M[1][v] = src[v * SW_TPB]; M[3][v] = src[(5 + v) * SW_TPB]; }
+        }
+      };
+      if (AXIS == 0) {
+        // lane - 4 computed the face below; the first cell of the tile takes the last cell of the previous step
+        if (cl == 0 && act && s >= 0) get(xs + 4 * (SW_CELLS - 1));
+        __syncwarp();
+        if (act) put();
+        __syncwarp();
+        if (cl > 0 && act && s >= 0) get(xs - 4);
+      } else {
+        if (act && s >= 0) get(xs);
+        if (act) put();
+      }
+    }
+    (void)NX;
+    if (act && s >= 0) {
+      // ---- Eq. 8-10 restricted to the two faces of this direction, S2O4 combine
+      double vol, Ap[3] = { 0, 0, 0 }, Am[3] = { 0, 0, 0 }, Sp = 0, Sm = 0, cf;
+      if (CART) { vol = m.h[0] * m.h[1] * m.h[2]; cf = 0.25 / m.h[AXIS]; }
+      else {
+        vol = m.met[MET_VOL * n + cur.cL];
+        // the cell below along AXIS owns the - face
+        int cm;
+        if (AXIS == 0) { const int i = cur.cL % m.ni; cm = (i == 0) ? cur.cL + m.ni - 1 : cur.cL - 1; }
+        else if (AXIS == 1) { const int ij = cur.cL % (int)m.plane; cm = (ij < m.ni) ? cur.cL + (int)m.plane - m.ni : cur.cL - m.ni; }
+        else { cm = (cur.cL < (int)m.plane) ? cur.cL + (int)(n - m.plane) : cur.cL - (int)m.plane; }
+#pragma unroll
+        for (int r = 0; r < 3; r++) { Ap[r] = m.met[(MET_AREA + 3 * AXIS + r) * n + cur.cL]; Am[r] = m.met[(MET_AREA + 3 * AXIS + r) * n + cm]; }
+        Sp = sqrt(Ap[0] * Ap[0] + Ap[1] * Ap[1] + Ap[2] * Ap[2]); Sm = sqrt(Am[0] * Am[0] + Am[1] * Am[1] + Am[2] * Am[2]);
+        cf = 0.25 / vol;
+      }
+      auto qsum = [&](double x) { x += __shfl_xor_sync(amask, x, 1); x += __shfl_xor_sync(amask, x, 2); return x; };
+      const double hdt = 0.5 * dt;
+      const double* rb = smr + par * (10 * SW_TPB) + tid;
+      const int comp = q - 1;      // gradient component owned by this lane (q = 0: the cell average)
+#pragma unroll
+      for (int v = 0; v < 5; v++) {
+        // sums over the four Gauss points of the face pair
+        double sF = 0, sFt, sV[3] = { 0, 0, 0 }, sD[3];
+        const double d1 = P[3][v] - M[3][v];
+        double d0 = 0;
+        if (!STAGE2) d0 = P[2][v] - M[2][v];
+        if (CART) {
+          sFt = qsum(P[1][v] - M[1][v]);
+          sD[0] = qsum(d1);
+          if (!STAGE2) { sF = qsum(P[0][v] - M[0][v]); sV[0] = qsum(d0); }
+        } else {
+          sFt = qsum(P[1][v] * Sp - M[1][v] * Sm);
+#pragma unroll
+          for (int r = 0; r < 3; r++) sD[r] = qsum(P[3][v] * Ap[r] - M[3][v] * Am[r]);
+          if (!STAGE2) {
+            sF = qsum(P[0][v] * Sp - M[0][v] * Sm);
+#pragma unroll
+            for (int r = 0; r < 3; r++) sV[r] = qsum(P[2][v] * Ap[r] - M[2][v] * Am[r]);
+          }
+        }
+        // this lane's component of the record { Q, G_x, G_y, G_z }
+        double gV = 0.0, gD = 0.0;      // gradient sums of the values / of the time derivatives, this lane's component
+        if (CART) { if (comp == AXIS) { gV = sV[0]; gD = sD[0]; } }
+        else {
+          if (comp == 0) { gV = sV[0]; gD = sD[0]; } else if (comp == 1) { gV = sV[1]; gD = sD[1]; } else if (comp == 2) { gV = sV[2]; gD = sD[2]; }
+        }
+        if (!STAGE2) {
+          double inc_star, inc_save;
+          if (q == 0) { inc_star = -cf * (hdt * sF + 0.125 * dt * dt * sFt); inc_save = -cf * (dt * sF + (1.0 / 6.0) * dt * dt * sFt); }
+          else { inc_star = cf * (gV + hdt * gD); inc_save = cf * gV; }
+          double b_star, b_save;
+          if (FIRST) { b_star = (q == 0) ? rb[v * SW_TPB] : 0.0; b_save = b_star; }
+          else { b_star = rb[v * SW_TPB]; b_save = rb[(5 + v) * SW_TPB]; }
+          Wstar[iQG(v, cur.cL, n) + q] = b_star + inc_star;
+          Wsave[iQG(v, cur.cL, n) + q] = b_save + inc_save;
+          Wstar[iD(v, cur.cL, n) + 4 * AXIS + q] = d0 + hdt * d1;
+          Wsave[iD(v, cur.cL, n) + 4 * AXIS + q] = d0;
+        } else {
+          const double inc = (q == 0) ? -cf * ((1.0 / 3.0) * dt * dt * sFt) : cf * (dt * gD);
+          Wsave[iQG(v, cur.cL, n) + q] = rb[v * SW_TPB] + inc;
+          Wsave[iD(v, cur.cL, n) + 4 * AXIS + q] = rb[(5 + v) * SW_TPB] + dt * d1;
+        }
+      }
+    }
+    line = nline; s = ns; cur = nxt; par ^= 1;
+  }
+}
+
+}  // namespace cgks
