@@ -46,6 +46,7 @@ struct cgks_ctx {
   int kofs = 0, nk_global = 0;          // global plane of local plane 0 (may be negative: wraps), planes of the global mesh
   int phase = 0;                        // sub-domain: 0 = next is stage 1 (input W[cur]), 1 = next is stage 2 (input W[star])
   int S = 0;                            // slab depth in k-planes; S == nk: whole mesh resident
+  int sweep_want = 32;                  // lines per warp the segmentation of the sweep kernels aims at
   int sweep_minseg = 24;                // shortest segment of a j / k line of the sweep kernels
   int split = 0;                        // 1: three-kernel pipeline (flux -> fx -> update) instead of the sweep kernels
   int slots_pv = 0, slots_fx = 0;
@@ -347,7 +348,7 @@ static void launch_sweeps(cgks_ctx* c, const Slab& sl, const double* Win, double
     const int len = ax == 1 ? m.nj : cnt;
     sp.seg = len; sp.nseg = 1;
     if (ax != 0) {
-      const long want = 32L * maxb * (SW_TPB / 32);
+      const long want = (long)c->sweep_want * maxb * (SW_TPB / 32);
       const long full = (long)sp.ntx * (ax == 1 ? cnt : m.nj);
       long nseg = (want + full - 1) / full; if (nseg < 1) nseg = 1;
       long seg = (len + nseg - 1) / nseg; if (seg < c->sweep_minseg) seg = c->sweep_minseg; if (seg > len) seg = len;

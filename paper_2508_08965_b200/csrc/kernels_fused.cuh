@@ -119,17 +119,19 @@ __global__ void __launch_bounds__(SW_TPB, FLUX_MINB) sweep_kernel(Mesh m, Slab s
       for (int c = 0; c < 10; c++) cp_async16(dst + (10 + c) * (2 * SW_TPB), pR + (long)(c >> 1) * (4 * sl.stride_pv) + 2 * (c & 1));
       if (s >= 0) {
         double* r = smr + par * (10 * SW_TPB) + tid;
+        const long oq = 4 * (long)p.cL + q, sq = 4 * n;
         if (FIRST) {
           if (q == 0) {
 #pragma unroll
-            for (int v = 0; v < 5; v++) cp_async8(r + v * SW_TPB, Wcur + iQG(v, p.cL, n));
+            for (int v = 0; v < 5; v++) cp_async8(r + v * SW_TPB, Wcur + oq + v * sq);
           }
         } else if (!STAGE2) {
 #pragma unroll
-          for (int v = 0; v < 5; v++) { cp_async8(r + v * SW_TPB, Wstar + iQG(v, p.cL, n) + q); cp_async8(r + (5 + v) * SW_TPB, Wsave + iQG(v, p.cL, n) + q); }
+          for (int v = 0; v < 5; v++) { cp_async8(r + v * SW_TPB, Wstar + oq + v * sq); cp_async8(r + (5 + v) * SW_TPB, Wsave + oq + v * sq); }
         } else {
+          const long od = 20 * n + 12 * (long)p.cL + 4 * AXIS + q, sd = 12 * n;
 #pragma unroll
-          for (int v = 0; v < 5; v++) { cp_async8(r + v * SW_TPB, Wsave + iQG(v, p.cL, n) + q); cp_async8(r + (5 + v) * SW_TPB, Wsave + iD(v, p.cL, n) + 4 * AXIS + q); }
+          for (int v = 0; v < 5; v++) { cp_async8(r + v * SW_TPB, Wsave + oq + v * sq); cp_async8(r + (5 + v) * SW_TPB, Wsave + od + v * sd); }
         }
       }
     }
@@ -153,27 +155,28 @@ __global__ void __launch_bounds__(SW_TPB, FLUX_MINB) sweep_kernel(Mesh m, Slab s
       WLg[v] = l0.x; gL[3 * v] = l0.y; gL[3 * v + 1] = l1.x; gL[3 * v + 2] = l1.y;
       WRg[v] = r0.x; gR[3 * v] = r0.y; gR[3 * v + 1] = r1.x; gR[3 * v + 2] = r1.y;
     }
-    // the step after this one (warp-uniform), its inputs stream in during the arithmetic of this one
+    // the step after this one (warp-uniform): its inputs stream in during the arithmetic of this one
     int nline = line, ns = s + 1;
     if (ns >= L.len) { nline = line + nw; ns = -1; if (nline < sp.nlines) L = sweep_line<AXIS>(m, sp, nline, cl); }
     SweepPos nxt; nxt.act = false; nxt.cL = 0; nxt.cR = 0; nxt.offL = 0; nxt.offR = 0;
     if (nline < sp.nlines) nxt = sweep_pos<AXIS>(m, sl, L, ns, cl);
     issue(nxt, ns, par ^ 1);
 
+    // Lanes without a cell (ragged last tile, the extra first face of an i-line) run the arithmetic on whatever their staging
+    // column holds and are masked at every global load and store: the warp stays converged, the shuffles need no mask logic.
     const bool act = cur.act;
-    const unsigned amask = __ballot_sync(0xffffffffu, act);
     double P[4][5];       // this face, global frame: F^n, F_t^n, own-side (left) value and time derivative
     double R[2][5];       // right-hand interface value and time derivative: they belong to the next cell
     double fr[3][3];
-    if (act) {
+    {
       // positivity (reading R9, point-wise): a non-physical reconstructed state falls back to the cell average
-      if (!admissible(WLg)) {
+      if (act && !admissible(WLg)) {
 #pragma unroll
         for (int c = 0; c < 5; c++) WLg[c] = Win[iQG(c, cur.cL, n)];
 #pragma unroll
         for (int c = 0; c < 15; c++) gL[c] = 0.0;
       }
-      if (!admissible(WRg)) {
+      if (act && !admissible(WRg)) {
 #pragma unroll
         for (int c = 0; c < 5; c++) WRg[c] = Win[iQG(c, cur.cR, n)];
 #pragma unroll
@@ -181,8 +184,8 @@ __global__ void __launch_bounds__(SW_TPB, FLUX_MINB) sweep_kernel(Mesh m, Slab s
       }
       double WL[5], WR[5], SL[3][5], SR[3][5];
       if (CART) {
-        const int p0 = AXIS, p1 = (AXIS + 1) % 3, p2 = (AXIS + 2) % 3;
-        const int pm[3] = { p0, p1, p2 };
+        // face frame = cyclic permutation of the axes: n = e_AXIS, t1 = e_(AXIS+1), t2 = e_(AXIS+2)
+        const int pm[3] = { AXIS, (AXIS + 1) % 3, (AXIS + 2) % 3 };
         WL[0] = WLg[0]; WL[4] = WLg[4]; WR[0] = WRg[0]; WR[4] = WRg[4];
 #pragma unroll
         for (int a = 0; a < 3; a++) { WL[1 + a] = WLg[1 + pm[a]]; WR[1 + a] = WRg[1 + pm[a]]; }
@@ -194,8 +197,9 @@ __global__ void __launch_bounds__(SW_TPB, FLUX_MINB) sweep_kernel(Mesh m, Slab s
         }
       } else {
         double A[3];
+        const long cg = act ? cur.cL : 0;
 #pragma unroll
-        for (int r = 0; r < 3; r++) { A[r] = m.met[(MET_AREA + 3 * AXIS + r) * n + cur.cL]; fr[1][r] = m.met[(MET_TAN + 3 * AXIS + r) * n + cur.cL]; }
+        for (int r = 0; r < 3; r++) { A[r] = m.met[(MET_AREA + 3 * AXIS + r) * n + cg]; fr[1][r] = m.met[(MET_TAN + 3 * AXIS + r) * n + cg]; }
         const double S = sqrt(A[0] * A[0] + A[1] * A[1] + A[2] * A[2]);
 #pragma unroll
         for (int r = 0; r < 3; r++) fr[0][r] = A[r] / S;
@@ -273,26 +277,30 @@ __global__ void __launch_bounds__(SW_TPB, FLUX_MINB) sweep_kernel(Mesh m, Slab s
       }
     }
     (void)NX;
-    if (act && s >= 0) {
+    if (s >= 0) {
       // ---- Eq. 8-10 restricted to the two faces of this direction, S2O4 combine
-      double vol, Ap[3] = { 0, 0, 0 }, Am[3] = { 0, 0, 0 }, Sp = 0, Sm = 0, cf;
-      if (CART) { vol = m.h[0] * m.h[1] * m.h[2]; cf = 0.25 / m.h[AXIS]; }
+      double Ap[3] = { 0, 0, 0 }, Am[3] = { 0, 0, 0 }, Sp = 0, Sm = 0, cf;
+      if (CART) cf = 0.25 / m.h[AXIS];
       else {
-        vol = m.met[MET_VOL * n + cur.cL];
+        const int cg = act ? cur.cL : 0;
         // the cell below along AXIS owns the - face
         int cm;
-        if (AXIS == 0) { const int i = cur.cL % m.ni; cm = (i == 0) ? cur.cL + m.ni - 1 : cur.cL - 1; }
-        else if (AXIS == 1) { const int ij = cur.cL % (int)m.plane; cm = (ij < m.ni) ? cur.cL + (int)m.plane - m.ni : cur.cL - m.ni; }
-        else { cm = (cur.cL < (int)m.plane) ? cur.cL + (int)(n - m.plane) : cur.cL - (int)m.plane; }
+        if (AXIS == 0) { const int i = cg % m.ni; cm = (i == 0) ? cg + m.ni - 1 : cg - 1; }
+        else if (AXIS == 1) { const int ij = cg % (int)m.plane; cm = (ij < m.ni) ? cg + (int)m.plane - m.ni : cg - m.ni; }
+        else { cm = (cg < (int)m.plane) ? cg + (int)(n - m.plane) : cg - (int)m.plane; }
 #pragma unroll
-        for (int r = 0; r < 3; r++) { Ap[r] = m.met[(MET_AREA + 3 * AXIS + r) * n + cur.cL]; Am[r] = m.met[(MET_AREA + 3 * AXIS + r) * n + cm]; }
+        for (int r = 0; r < 3; r++) { Ap[r] = m.met[(MET_AREA + 3 * AXIS + r) * n + cg]; Am[r] = m.met[(MET_AREA + 3 * AXIS + r) * n + cm]; }
         Sp = sqrt(Ap[0] * Ap[0] + Ap[1] * Ap[1] + Ap[2] * Ap[2]); Sm = sqrt(Am[0] * Am[0] + Am[1] * Am[1] + Am[2] * Am[2]);
-        cf = 0.25 / vol;
+        cf = 0.25 / m.met[MET_VOL * n + cg];
       }
-      auto qsum = [&](double x) { x += __shfl_xor_sync(amask, x, 1); x += __shfl_xor_sync(amask, x, 2); return x; };
+      auto qsum = [&](double x) { x += __shfl_xor_sync(0xffffffffu, x, 1); x += __shfl_xor_sync(0xffffffffu, x, 2); return x; };
       const double hdt = 0.5 * dt;
       const double* rb = smr + par * (10 * SW_TPB) + tid;
       const int comp = q - 1;      // gradient component owned by this lane (q = 0: the cell average)
+      // this lane's component of the records of variable 0; the next variable is 4 n (records) / 12 n (line differences) further
+      const long oq = 4 * (long)cur.cL + q, od = 20 * n + 12 * (long)cur.cL + 4 * AXIS + q;
+      double* pq_star = Wstar + oq; double* pq_save = Wsave + oq; double* pd_star = Wstar + od; double* pd_save = Wsave + od;
+      const long sq = 4 * n, sd = 12 * n;
 #pragma unroll
       for (int v = 0; v < 5; v++) {
         // sums over the four Gauss points of the face pair
@@ -327,14 +335,18 @@ __global__ void __launch_bounds__(SW_TPB, FLUX_MINB) sweep_kernel(Mesh m, Slab s
           double b_star, b_save;
           if (FIRST) { b_star = (q == 0) ? rb[v * SW_TPB] : 0.0; b_save = b_star; }
           else { b_star = rb[v * SW_TPB]; b_save = rb[(5 + v) * SW_TPB]; }
-          Wstar[iQG(v, cur.cL, n) + q] = b_star + inc_star;
-          Wsave[iQG(v, cur.cL, n) + q] = b_save + inc_save;
-          Wstar[iD(v, cur.cL, n) + 4 * AXIS + q] = d0 + hdt * d1;
-          Wsave[iD(v, cur.cL, n) + 4 * AXIS + q] = d0;
+          if (act) {
+            pq_star[v * sq] = b_star + inc_star;
+            pq_save[v * sq] = b_save + inc_save;
+            pd_star[v * sd] = d0 + hdt * d1;
+            pd_save[v * sd] = d0;
+          }
         } else {
           const double inc = (q == 0) ? -cf * ((1.0 / 3.0) * dt * dt * sFt) : cf * (dt * gD);
-          Wsave[iQG(v, cur.cL, n) + q] = rb[v * SW_TPB] + inc;
-          Wsave[iD(v, cur.cL, n) + 4 * AXIS + q] = rb[(5 + v) * SW_TPB] + dt * d1;
+          if (act) {
+            pq_save[v * sq] = rb[v * SW_TPB] + inc;
+            pd_save[v * sd] = rb[(5 + v) * SW_TPB] + dt * d1;
+          }
         }
       }
     }
