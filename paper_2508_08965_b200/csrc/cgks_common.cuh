@@ -6,10 +6,11 @@
 namespace cgks {
 
 // ---- HBM layout (all fp64, structure-of-arrays, i fastest) ---------------------------------------------------------
-// state buffer        80 N doubles: [5][N][4] records { Q_v, G_v (3) } (32 B), then [5][N][12] records D_v (96 B).  A neighbour's
-//                     average and gradient arrive with ONE 256-bit load (one 32-byte sector), a cell's 12 line differences with
-//                     three, and the update writes them with as many stores: 22 loads per (cell, variable) in the
-//                     reconstruction instead of 85 with one plane per component.
+// state buffer        80 N doubles: [5][N][4] records { Q_v, G_v (3) } (32 B), then [5][3][N][4] records of the four line
+//                     differences D_v of one axis (32 B).  A neighbour's average and gradient arrive with ONE 256-bit load
+//                     (one 32-byte sector), a cell's 12 line differences with three: 22 loads per (cell, variable) in the
+//                     reconstruction instead of 85 with one plane per component; a sweep kernel (kernels_fused.cuh) touches
+//                     exactly the record of its own axis, contiguous from cell to cell.
 // metrics (general)   [37][N]      J0 3r+a (0..8) | J0^-1 9+3a+r... see MET_* | vol | +face vector areas | +face tangents
 // pv (slab)           [24*5][slots*plane][4]   record (point p = 4m+q, variable v, cell slot) = { value, physical gradient (3) }
 // fx (slab)           [360][slots*plane]   plane (4ax+q)*30 + c : Fn 0..4 | Ft 5..9 | VL 10..14 | DL 15..19 | VR 20..24 | DR 25..29
@@ -17,12 +18,13 @@ enum { NVAR = 5, NSTATE = 80, NPV = 480, NFX = 360, NMET = 37 };
 enum { MET_J0 = 0, MET_J0INV = 9, MET_VOL = 18, MET_AREA = 19, MET_TAN = 28 };
 // index of the first double of the records of (variable v, cell c) in a state buffer of n cells
 __host__ __device__ inline long iQG(int v, long c, long n) { return ((long)v * n + c) * 4; }             // + 0: Q, + 1 + r: G_r
-__host__ __device__ inline long iD(int v, long c, long n) { return 20 * n + ((long)v * n + c) * 12; }   // + s: D_s
+__host__ __device__ inline long iD(int v, int ax, long c, long n) { return 20 * n + ((long)(3 * v + ax) * n + c) * 4; }   // + q: D_(4 ax + q)
 // field number f = 0..79 in the user order (Q v | G 5+3v+r | D 20+12v+s) -> index in the state buffer
 __host__ __device__ inline long iField(int f, long c, long n) {
   if (f < 5) return iQG(f, c, n);
   if (f < 20) return iQG((f - 5) / 3, c, n) + 1 + (f - 5) % 3;
-  return iD((f - 20) / 12, c, n) + (f - 20) % 12;
+  const int s = (f - 20) % 12;
+  return iD((f - 20) / 12, s / 4, c, n) + s % 4;
 }
 
 struct Mesh {

@@ -129,7 +129,7 @@ __global__ void __launch_bounds__(SW_TPB, FLUX_MINB) sweep_kernel(Mesh m, Slab s
 #pragma unroll
           for (int v = 0; v < 5; v++) { cp_async8(r + v * SW_TPB, Wstar + oq + v * sq); cp_async8(r + (5 + v) * SW_TPB, Wsave + oq + v * sq); }
         } else {
-          const long od = 20 * n + 12 * (long)p.cL + 4 * AXIS + q, sd = 12 * n;
+          const long od = iD(0, AXIS, p.cL, n) + q, sd = 12 * n;
 #pragma unroll
           for (int v = 0; v < 5; v++) { cp_async8(r + v * SW_TPB, Wsave + oq + v * sq); cp_async8(r + (5 + v) * SW_TPB, Wsave + od + v * sd); }
         }
@@ -298,7 +298,7 @@ __global__ void __launch_bounds__(SW_TPB, FLUX_MINB) sweep_kernel(Mesh m, Slab s
       const double* rb = smr + par * (10 * SW_TPB) + tid;
       const int comp = q - 1;      // gradient component owned by this lane (q = 0: the cell average)
       // this lane's component of the records of variable 0; the next variable is 4 n (records) / 12 n (line differences) further
-      const long oq = 4 * (long)cur.cL + q, od = 20 * n + 12 * (long)cur.cL + 4 * AXIS + q;
+      const long oq = 4 * (long)cur.cL + q, od = iD(0, AXIS, cur.cL, n) + q;
       double* pq_star = Wstar + oq; double* pq_save = Wsave + oq; double* pd_star = Wstar + od; double* pd_save = Wsave + od;
       const long sq = 4 * n, sd = 12 * n;
 #pragma unroll

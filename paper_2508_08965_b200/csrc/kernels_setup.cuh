@@ -132,7 +132,6 @@ __global__ void set_state_kernel(Mesh m, const double* __restrict__ Qin, const d
   const int i = (int)(c % m.ni), j = (int)((c / m.ni) % m.nj), k = (int)(c / m.plane);
   const double* q = Qin + (long)v * m.n;
   double* qg = W + iQG(v, c, m.n);
-  double* dd = W + iD(v, c, m.n);
   qg[0] = q[c];
   double dr[3] = { 0, 0, 0 };
   if (Gin == nullptr || Din == nullptr) {
@@ -157,10 +156,10 @@ __global__ void set_state_kernel(Mesh m, const double* __restrict__ Qin, const d
   }
   if (Din != nullptr) {
 #pragma unroll
-    for (int s = 0; s < 12; s++) dd[s] = Din[(long)(12 * v + s) * m.n + c];
+    for (int s = 0; s < 12; s++) W[iD(v, s / 4, c, m.n) + s % 4] = Din[(long)(12 * v + s) * m.n + c];
   } else {
 #pragma unroll
-    for (int s = 0; s < 12; s++) dd[s] = dr[s / 4];
+    for (int s = 0; s < 12; s++) W[iD(v, s / 4, c, m.n) + s % 4] = dr[s / 4];
   }
 }
 
@@ -170,10 +169,9 @@ __global__ void get_state_kernel(Mesh m, const double* __restrict__ W, double* _
   if (c >= m.n) return;
   const int v = blockIdx.y;
   const double* qg = W + iQG(v, c, m.n);
-  const double* dd = W + iD(v, c, m.n);
   if (Qo) Qo[(long)v * m.n + c] = qg[0];
   if (Go) for (int r = 0; r < 3; r++) Go[(long)(3 * v + r) * m.n + c] = qg[1 + r];
-  if (Do) for (int s = 0; s < 12; s++) Do[(long)(12 * v + s) * m.n + c] = dd[s];
+  if (Do) for (int s = 0; s < 12; s++) Do[(long)(12 * v + s) * m.n + c] = W[iD(v, s / 4, c, m.n) + s % 4];
 }
 
 // time step (reading S3): dt = min over cells of cfl / sum_d (|U.n_d| + c)/h_d and of the viscous cap.
@@ -239,14 +237,13 @@ __global__ void cfl_kernel(Mesh m, const double* __restrict__ W, CflPrm p, unsig
 // buffer W [80][n] and a contiguous buffer [80][np][plane].  PACK: W -> buf, else buf -> W.
 template <bool PACK>
 __global__ void halo_kernel(double* __restrict__ W, double* __restrict__ buf, long n, long plane, int kfirst, int np) {
-  // per variable the planes [kfirst, kfirst + np) are one contiguous run of 4 np plane doubles (Q, G records) and one of
-  // 12 np plane doubles (D records); the buffer holds the five Q/G runs, then the five D runs
-  const long runA = 4L * np * plane, runB = 12L * np * plane;
-  const long tot = 5 * (runA + runB);
+  // the planes [kfirst, kfirst + np) of every record array (5 of { Q, G }, 15 of the line differences of one axis) are one
+  // contiguous run of 4 np plane doubles; the buffer holds the 20 runs one after the other
+  const long run = 4L * np * plane;
+  const long tot = 20 * run;
   for (long t = (long)blockIdx.x * blockDim.x + threadIdx.x; t < tot; t += (long)gridDim.x * blockDim.x) {
-    double* w;
-    if (t < 5 * runA) { const long v = t / runA, r = t - v * runA; w = W + iQG((int)v, (long)kfirst * plane, n) + r; }
-    else { const long u = t - 5 * runA, v = u / runB, r = u - v * runB; w = W + iD((int)v, (long)kfirst * plane, n) + r; }
+    const int a = (int)(t / run); const long r = t - a * run;
+    double* w = W + (a < 5 ? iQG(a, (long)kfirst * plane, n) : iD((a - 5) / 3, (a - 5) % 3, (long)kfirst * plane, n)) + r;
     if (PACK) buf[t] = *w; else *w = buf[t];
   }
 }

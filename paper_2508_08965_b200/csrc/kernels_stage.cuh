@@ -121,13 +121,12 @@ __global__ void __launch_bounds__(128, 3) recon_kernel(Mesh m, Slab sl, const do
   recon_gather_axis<CART, 1>(rc, ii, jj, kk, q0, a, dface);
   recon_gather_axis<CART, 2>(rc, ii, jj, kk, q0, a, dface);
   {   // line differences (Eq. 10): raw D, the factor h3' is folded into the coefficients; three 256-bit loads
-    const double* dd = W + iD(v, x.c, n);
     double Dl[4];
-    ld4_ro(dd, Dl[0], Dl[1], Dl[2], Dl[3]);
+    ld4_ro(W + iD(v, 0, x.c, n), Dl[0], Dl[1], Dl[2], Dl[3]);
     la[0] = 0.25 * (Dl[0] + Dl[1] + Dl[2] + Dl[3]); acc_line<0>(Dl, a);
-    ld4_ro(dd + 4, Dl[0], Dl[1], Dl[2], Dl[3]);
+    ld4_ro(W + iD(v, 1, x.c, n), Dl[0], Dl[1], Dl[2], Dl[3]);
     la[1] = 0.25 * (Dl[0] + Dl[1] + Dl[2] + Dl[3]); acc_line<1>(Dl, a);
-    ld4_ro(dd + 8, Dl[0], Dl[1], Dl[2], Dl[3]);
+    ld4_ro(W + iD(v, 2, x.c, n), Dl[0], Dl[1], Dl[2], Dl[3]);
     la[2] = 0.25 * (Dl[0] + Dl[1] + Dl[2] + Dl[3]); acc_line<2>(Dl, a);
   }
   double chi = 1.0;
@@ -501,9 +500,9 @@ __global__ void __launch_bounds__(128) update_kernel(Mesh m, Slab sl, const doub
     const double hdt = 0.5 * dt;
     st4(Wstar + iQG(v, x.c, n), qn + hdt * L + 0.125 * dt * dt * Lt, SG0[0] + hdt * SG1[0], SG0[1] + hdt * SG1[1], SG0[2] + hdt * SG1[2]);
     st4(Wsave + iQG(v, x.c, n), qn + dt * L + (1.0 / 6.0) * dt * dt * Lt, SG0[0], SG0[1], SG0[2]);
-    double* ds = Wstar + iD(v, x.c, n); double* dv = Wsave + iD(v, x.c, n);
 #pragma unroll
     for (int s = 0; s < 12; s += 4) {
+      double* ds = Wstar + iD(v, s / 4, x.c, n) - s; double* dv = Wsave + iD(v, s / 4, x.c, n) - s;
       st4(ds + s, SD0[s] + hdt * SD1[s], SD0[s + 1] + hdt * SD1[s + 1], SD0[s + 2] + hdt * SD1[s + 2], SD0[s + 3] + hdt * SD1[s + 3]);
       st4(dv + s, SD0[s], SD0[s + 1], SD0[s + 2], SD0[s + 3]);
     }
@@ -512,9 +511,9 @@ __global__ void __launch_bounds__(128) update_kernel(Mesh m, Slab sl, const doub
     double a0, a1, a2, a3;
     ld4(qg, a0, a1, a2, a3);
     st4(qg, a0 + (1.0 / 3.0) * dt * dt * Lt, a1 + dt * SG1[0], a2 + dt * SG1[1], a3 + dt * SG1[2]);
-    double* dv = Wsave + iD(v, x.c, n);
 #pragma unroll
     for (int s = 0; s < 12; s += 4) {
+      double* dv = Wsave + iD(v, s / 4, x.c, n) - s;
       ld4(dv + s, a0, a1, a2, a3);
       st4(dv + s, a0 + dt * SD1[s], a1 + dt * SD1[s + 1], a2 + dt * SD1[s + 2], a3 + dt * SD1[s + 3]);
     }
