@@ -3,7 +3,7 @@
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--n 384] [--impl ours|reference] [--parallel replicas|slab]
 
-One "step" = cgks_compute_dt + cgks_step (two stages: reconstruction, GENO blend, gas-kinetic flux, update/combine)
+One "step" = cgks_compute_dt + cgks_step (two stages: reconstruction + GENO blend, then three sweep kernels: gas-kinetic flux with update/combine)
 over the whole mesh.  Workload at N = 1: BASELINE.json configs[4], supersonic isotropic turbulence Ma_t = 1 on the
 periodic Cartesian 384^3 mesh (synthetic, seeded).  north_star asks for one GPU, so by default
 --gpus N runs N independent replicas (weak scaling, no collective); --parallel slab runs the paper's own parallelisation
@@ -25,27 +25,29 @@ sys.path.insert(0, ROOT)
 
 METRIC = "cell-updates/s per S2O4 step (fp64)"
 UNIT = "cell-updates/s"
-# Dominant kernel = gas-kinetic flux (flux_kernel), bound by the plain FP64 ALUs.  Two flop counts per face Gauss point
-# (FMA = 2, add/mul = 1), DESIGN.md section 7.2:
-#  * EXECUTED by the formulation as built (primed-basis moments, own reciprocal / rsqrt / exp / erfc of csrc/fastmath64.cuh),
-#    from ncu's executed-FP64-op counters on the committed capture profiles/r02d_kernels_128.md: stage 1 computes F, F_t,
-#    Q, Q_t and both one-sided values, stage 2 only the time derivatives.  This is the leanest formulation known to the
-#    authors of this repository and is what `roofline.achieved` uses: it can only understate the algorithmic work.
+# Dominant kernel = sweep_kernel (gas-kinetic flux + update/S2O4 combine of one face direction, csrc/kernels_fused.cuh), bound by
+# the plain FP64 ALUs.  Two flop counts per face Gauss point (FMA = 2, add/mul = 1), DESIGN.md section 7.2:
+#  * EXECUTED by the formulation as built (primed-basis moments, own reciprocal / rsqrt / exp / erfc of csrc/fastmath64.cuh, the
+#    quad sums and the combine), from ncu's executed-FP64-op counters on the committed capture profiles/r02f_kernels_128.md,
+#    per point of an updated cell (the extra first face of every line of a sweep is NOT counted as useful work): stage 1
+#    computes F, F_t, Q, Q_t and both one-sided values, stage 2 only the time derivatives.  This is the leanest formulation
+#    known to the authors of this repository and is what `roofline.achieved` uses: it can only understate the algorithmic work.
 #  * ORACLE-COUNTED (counting-double build of the CPU oracle, oracle/flop_count.py; operations on non-zero
-#    operands): the oracle evaluates every term of Eq. 5 with the generic moment routine and needs 5x the arithmetic, so
+#    operands): the oracle evaluates every term of Eq. 5 with the generic moment routine and needs 7x the arithmetic, so
 #    a fraction formed with it exceeds 1; it is printed beside the other, not used as the numerator.
-FLUX_FLOPS_STAGE1 = 2176.0          # 820.4 DFMA + 443.8 DMUL + 91.3 DADD per point
-FLUX_FLOPS_STAGE2 = 2025.0          # 758.5 DFMA + 422.8 DMUL + 85.3 DADD per point
+SWEEP_FLOPS_STAGE1 = 2284.0         # per point: 832 DFMA + 458 DMUL + 161 DADD (flux solver 2176, quad sums and combine 108)
+SWEEP_FLOPS_STAGE2 = 2082.0         # per point: 761 DFMA + 441 DMUL + 118 DADD (flux solver 2025, quad sums and combine 57)
 FLUX_SOURCE_SHA16 = "e8b455be08183f62"      # sha256 (16 hex digits) of gks_flux.cuh + fastmath64.cuh + math_gen.cuh the counts were taken on
 FLUX_FLOPS_ORACLE = 15584.0          # tests/test_abi.py checks this constant against oracle/flop_count.py
-# Round 1's kernel executed 3092.7 / 2923.2 flops per point for the same result (profiles/r01d_kernels_128.md); VERDICT r1's
+# Round 1's flux kernel executed 3092.7 / 2923.2 flops per point for the same result (profiles/r01d_kernels_128.md); VERDICT r1's
 # target "frac >= 0.50, i.e. flux <= 223 ms per step" is stated in that count, so the fraction in that count is printed too.
 FLUX_FLOPS_R01 = (3092.7, 2923.2)
-FLUX_FP64_PIPE_ACTIVE_NCU = (0.630, 0.650)      # sm__pipe_fp64_cycles_active of the stage-1 / stage-2 launches, same capture
-# DRAM bytes per point of the same capture (dram__bytes_read + write per launch / points): the algorithmic bytes are
-# 40 inputs + 30 (stage 1) or 15 (stage 2) outputs of 8 B = 560 / 440 B
-FLUX_TRAFFIC_STAGE1 = 554.9
-FLUX_TRAFFIC_STAGE2 = 437.0
+SWEEP_FP64_PIPE_ACTIVE_NCU = (0.570, 0.586)     # sm__pipe_fp64_cycles_active of the stage-1 / stage-2 launches, same capture
+# Bytes per point.  Algorithmic: 2 x 20 reconstructed inputs (320 B) + the state records the direction reads and writes, per
+# cell and stage 1: 40 (Q^n) + 2 x 320 read, 3 x 640 written; stage 2: 3 x 320 read, 3 x 320 written; / 12 points.
+# Measured: dram__bytes_read + write per launch / points, same capture.
+SWEEP_BYTES_ALG = (320.0 + (40 + 640 + 1920) / 12.0, 320.0 + (960 + 960) / 12.0)
+SWEEP_TRAFFIC = (557.0, 480.0)
 FP64_PEAK_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12      # SMs x FP64 FMA lanes x 2 x max SM clock = 37.2
 
 
@@ -269,38 +271,55 @@ def run_ours(args):
                        "runs one full S2O4 step and ships Q back; the 75 derivative dof per cell (G, D) are NOT shipped: they are "
                        "re-bootstrapped from Q on the device (DESIGN.md reading S2) and not returned, so this is a cold-start step "
                        "(the full 80-dof state would be 36.2 GB each way at 384^3, i.e. PCIe-bound at ~1.5 s per step)"}
-    # ---- roofline of the dominant kernel (gas-kinetic flux) ---------------------------------------------------------
+    # ---- roofline of the dominant kernel (sweep_kernel: gas-kinetic flux + update, one launch per face direction) ----------
     peak_meas = binding.fp64_peak_tflops(dev) if rank == 0 else None
     fms, fnl = kms["flux"]
+    rms, rnl = kms["recon"]
     roof = None
     if fnl > 0:
-        # every flux launch covers 4 Gauss points of one face direction of its cells; summed over the launches of the
-        # profiled steps the points are 12 per cell per stage (+ the recomputed halo plane of each slab, counted in fnl)
-        pts_per_stage = 12 * cells_rank * slab_overhead(solver, nk_own if use_slab else n, use_slab)
-        flops = (FLUX_FLOPS_STAGE1 + FLUX_FLOPS_STAGE2) * pts_per_stage * psteps
+        # summed over the launches of the profiled steps the useful points are 12 per cell per stage (the extra first face of
+        # every line of a sweep is redundant work and not counted)
+        pts_per_stage = 12 * cells_rank
+        flops = (SWEEP_FLOPS_STAGE1 + SWEEP_FLOPS_STAGE2) * pts_per_stage * psteps
         ach = flops / (fms * 1e-3) / 1e12
         pts_per_launch = 2 * pts_per_stage * psteps / fnl
-        roof = {"bound": "alu", "kernel": "flux_kernel", "achieved": ach, "peak": FP64_PEAK_NOMINAL_TFLOPS, "unit": "TFLOP/s",
+        sm_mhz = clocks.get("sm_mhz") or 1965.0
+        # reconstruction: HBM-bound, 640 B read + 3840 B written per cell (+ the two extra planes of every slab)
+        nchunks = 1 if solver_slab(solver) >= (nk_own + 4 if use_slab else n) else math.ceil((nk_own if use_slab else n) / solver_slab(solver))
+        planes = (nk_own if use_slab else n) + (2 * nchunks if (use_slab or nchunks > 1) else 0)
+        recon_bytes = 2 * psteps * 4480.0 * planes * n * n
+        hbm_peak = measured_hbm_peak()
+        roof = {"bound": "alu", "kernel": "sweep_kernel", "achieved": ach, "peak": FP64_PEAK_NOMINAL_TFLOPS, "unit": "TFLOP/s",
                 "frac": ach / FP64_PEAK_NOMINAL_TFLOPS,
-                "flops_per_point_executed": [FLUX_FLOPS_STAGE1, FLUX_FLOPS_STAGE2],
+                "frac_at_measured_clock": ach / (FP64_PEAK_NOMINAL_TFLOPS * sm_mhz / 1965.0),
+                "flops_per_point_executed": [SWEEP_FLOPS_STAGE1, SWEEP_FLOPS_STAGE2],
                 "flops_per_point_oracle_counted": FLUX_FLOPS_ORACLE,
-                "achieved_with_oracle_count": ach * 2.0 * FLUX_FLOPS_ORACLE / (FLUX_FLOPS_STAGE1 + FLUX_FLOPS_STAGE2),
-                "frac_with_r01_flop_count": ach * sum(FLUX_FLOPS_R01) / (FLUX_FLOPS_STAGE1 + FLUX_FLOPS_STAGE2) / FP64_PEAK_NOMINAL_TFLOPS,
-                "fp64_pipe_active_ncu": list(FLUX_FP64_PIPE_ACTIVE_NCU),
-                "flops_note": "achieved = flops EXECUTED by this kernel's own (leanest known) formulation / time, so a leaner formulation lowers it "
-                              "at equal pipe utilisation (round 1 executed 42 % more flops per point); the CPU oracle's term-by-term evaluation "
-                              "needs 7x the arithmetic, so its count would give a fraction above 1; frac_with_r01_flop_count is the figure "
-                              "comparable with VERDICT r1's target (DESIGN.md 7.2)",
-                "traffic": 0.5 * (FLUX_TRAFFIC_STAGE1 + FLUX_TRAFFIC_STAGE2) * pts_per_launch,
-                "traffic_note": "bytes per average launch = ncu dram bytes per point (profiles/r02d_kernels_128.md) x points per launch; "
-                                "algorithmic bytes per point 560 (stage 1) / 440 (stage 2)",
+                "achieved_with_oracle_count": ach * 2.0 * FLUX_FLOPS_ORACLE / (SWEEP_FLOPS_STAGE1 + SWEEP_FLOPS_STAGE2),
+                "frac_with_r01_flop_count": ach * sum(FLUX_FLOPS_R01) / (SWEEP_FLOPS_STAGE1 + SWEEP_FLOPS_STAGE2) / FP64_PEAK_NOMINAL_TFLOPS,
+                "fp64_pipe_active_ncu": list(SWEEP_FP64_PIPE_ACTIVE_NCU),
+                "flops_note": "achieved = flops EXECUTED by this kernel's own (leanest known) formulation per useful point / time, so a leaner "
+                              "formulation lowers it at equal pipe utilisation (round 1's flux kernel executed 42 % more flops per point for "
+                              "the same result); 36 % of its FP64 instructions are DMUL/DADD, which occupy an FMA slot for one flop: at 100 % "
+                              "pipe activity this instruction mix reaches 0.79 of the FMA peak; the peak assumes the maximum SM clock, the "
+                              "box runs below it under its 1 kW power cap (frac_at_measured_clock uses the sampled clock); the CPU oracle's "
+                              "term-by-term evaluation needs 7x the arithmetic, so its count would give a fraction above 1 (DESIGN.md 7.2)",
+                "traffic": 0.5 * sum(SWEEP_TRAFFIC) * pts_per_launch,
+                "algorithmic_bytes": 0.5 * sum(SWEEP_BYTES_ALG) * pts_per_launch,
+                "traffic_note": "bytes per average launch = ncu dram bytes per point (profiles/r02f_kernels_128.md) x points per launch; "
+                                "algorithmic bytes per point %.0f (stage 1) / %.0f (stage 2)" % SWEEP_BYTES_ALG,
+                "hbm_frac_of_this_kernel": (0.5 * sum(SWEEP_BYTES_ALG) * pts_per_launch / (fms / fnl * 1e-3) / 1e9) / hbm_peak[0],
                 "peak_source": "derived: 148 SMs x 64 FP64 FMA lanes x 2 x 1.965 GHz (DESIGN.md section 7); "
                                "MEASURED_PEAKS.json has no FP64 entry",
                 "peak_dfma_microbench": peak_meas, "frac_of_dfma_microbench": (ach / peak_meas) if peak_meas else None,
                 "avg_launch_ms": fms / fnl, "launches": fnl,
                 "share_of_step": fms / (pms if pms > 0 else 1.0),
                 "kernel_ms_per_step": {k: v[0] / psteps for k, v in kms.items()},
-                "profiled_steps": psteps, "profiled_ms_per_step": pms / psteps}
+                "profiled_steps": psteps, "profiled_ms_per_step": pms / psteps,
+                "other_kernels": {"recon_kernel": {
+                    "bound": "hbm", "achieved": recon_bytes / (rms * 1e-3) / 1e9 if rms > 0 else None, "peak": hbm_peak[0], "unit": "GB/s",
+                    "frac": (recon_bytes / (rms * 1e-3) / 1e9 / hbm_peak[0]) if rms > 0 else None, "peak_source": hbm_peak[1],
+                    "algorithmic_bytes_per_cell": 4480.0, "avg_launch_ms": rms / rnl if rnl else None, "launches": rnl,
+                    "share_of_step": rms / (pms if pms > 0 else 1.0)}}}
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
             "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "strong" if use_slab and world > 1 else "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
@@ -316,6 +335,15 @@ def run_ours(args):
         print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
+
+
+def measured_hbm_peak():
+    """(GB/s, source): the driver-written copy bandwidth of this pool's B200s, else the profiling guide's fallback."""
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs"
+    except Exception:
+        return 6650.0, "fallback of /opt/skills/guides/B200_PROFILING.md (no MEASURED_PEAKS.json)"
 
 
 def solver_slab(solver):

@@ -247,6 +247,10 @@ class Solver:
     def launch_count(self):
         return int(lib().cgks_launch_count(self._h))
 
+    def slab_depth(self):
+        """k-planes per chunk of the stage pipeline chosen from the workspace size (nk: whole mesh resident)."""
+        return int(lib().cgks_slab_depth(self._h))
+
     def set_profiling(self, on):
         self._check(lib().cgks_set_profiling(self._h, int(on)))
 

@@ -74,6 +74,9 @@ extern "C" const char* cgks_last_error(const cgks_ctx* c) { return c ? c->err.c_
 extern "C" long cgks_launch_count(const cgks_ctx* c) { return c ? c->launches : 0; }
 extern "C" int cgks_slab_depth(const cgks_ctx* c) { return c ? c->S : 0; }
 
+// CGKS_PIPELINE=split in the environment selects the three-kernel pipeline of rounds 1-2 (A/B timing, test taps)
+static bool pipeline_split() { const char* e = getenv("CGKS_PIPELINE"); return e && strcmp(e, "split") == 0; }
+
 static size_t fixed_bytes(long n, bool with_metrics) {
   size_t b = 3 * state_bytes(n) + align_up((size_t)5 * n * 8) + align_up(64);
   if (with_metrics) b += align_up((size_t)NMET * n * 8);
@@ -84,16 +87,20 @@ extern "C" int cgks_workspace_bytes(int ni, int nj, int nk, size_t budget, size_
   if (ni < 4 || nj < 4 || nk < 4 || !bytes) return CGKS_EINVAL;
   const long plane = (long)ni * nj, n = plane * nk;
   const size_t fixed = fixed_bytes(n, true);
-  const size_t full = (size_t)nk * slot_bytes(plane);           // whole mesh resident
-  size_t slab = full;
+  // slab buffers: reconstructed face values only (sweep pipeline), + face fluxes in the three-kernel pipeline
+  const size_t sb = pipeline_split() ? slot_bytes(plane) : slot_bytes_pv(plane);
+  const size_t full_tap = (size_t)nk * slot_bytes(plane);       // whole mesh resident, with the face-flux buffer of the test tap
+  const size_t full = (size_t)nk * sb;                          // whole mesh resident
+  size_t slab = full_tap;
   const size_t cap = budget ? (budget > fixed ? budget - fixed : 0) : DEFAULT_SLAB_BYTES;
+  if (slab > cap) slab = full;
   if (slab > cap) {
-    long S = (long)(cap / slot_bytes(plane)) - 2;
+    long S = (long)(cap / sb) - 2;
     if (S < 2) {
       if (budget) return CGKS_ENOMEM;                           // not even a slab of two k-planes fits under the budget
       S = 2;
     }
-    slab = (size_t)(S + 2) * slot_bytes(plane);
+    slab = (size_t)(S + 2) * sb;
   }
   *bytes = fixed + align_up(slab) + ALIGN;
   return CGKS_OK;
@@ -164,7 +171,7 @@ static int create_impl(cgks_ctx** out, int ni, int nj, int nkg, int nk, int kofs
   cgks_ctx* c = new cgks_ctx();
   c->prm = *params; c->stream = (cudaStream_t)stream;
   c->open_k = open_k; c->kofs = kofs; c->nk_global = nkg;
-  { const char* e = getenv("CGKS_PIPELINE"); c->split = (e && strcmp(e, "split") == 0) ? 1 : 0; }
+  c->split = pipeline_split() ? 1 : 0;
   {
     int dev = 0; cudaGetDevice(&dev);
     if (cudaDeviceGetAttribute(&c->nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || c->nsm <= 0) c->nsm = 148;
@@ -226,6 +233,10 @@ static int create_impl(cgks_ctx** out, int ni, int nj, int nkg, int nk, int kofs
       long S = slots - 2;
       if (S < 2) { bail(CGKS_ENOMEM, "workspace too small for a slab of two k-planes"); break; }
       if (S > nk) S = nk;
+      {   // equal chunks: the same number of chunks, none of them a short remainder
+        const long owned = open_k ? nk - 4 : nk, nch = (owned + S - 1) / S;
+        S = (owned + nch - 1) / nch;
+      }
       c->S = (int)S; c->slots_pv = (int)S + 2; c->slots_fx = (int)S + 1;
     }
     c->pv = (double*)p; p += (size_t)NPV * c->slots_pv * m.plane * 8;

@@ -152,11 +152,61 @@ def test_slab_pipeline_equals_resident():
     full, _ = parity.run_gpu(w, 2)
     n = 12 ** 3
     fixed = 3 * 80 * n * 8 + 5 * n * 8 + 37 * n * 8 + 4096
-    budget = fixed + 6 * (480 + 360) * 144 * 8           # 6 slots -> slab depth 4 -> 3 chunks
+    budget = fixed + 6 * 480 * 144 * 8                   # 6 slots of reconstructed face values -> slab depth 4 -> 3 chunks
+    s = binding.Solver(w["nodes"], binding.make_params(**w["params"], nonlinear=1), budget_bytes=budget)
+    assert s.slab_depth() == 4
+    s.close()
     slab, _ = parity.run_gpu(w, 2, budget_bytes=budget)
     for a, b in zip(full, slab):
         assert np.array_equal(a, b)
     _check(w, 2, TOL_1 * 2, budget=budget)
+
+
+@pytest.mark.parametrize("case", ["tgv_curv", "iso_sup", "ragged", "jump"])
+def test_sweep_pipeline_against_the_three_kernel_pipeline(case, monkeypatch):
+    """The product path does flux + update in one sweep kernel per face direction (csrc/kernels_fused.cuh); the
+    three-kernel pipeline of rounds 1-2 (flux -> face-flux buffer -> update, CGKS_PIPELINE=split) is kept for A/B timing.
+    They order the sums of Eq. 8-9 differently (direction by direction and Gauss-point quads against face by face), so
+    they agree to round-off, not bit for bit; both match the oracle at 1e-10 per step."""
+    if case == "ragged":
+        nodes = inputs.cartesian_nodes((13, 9, 7), 0.0, 2.0 * np.pi); nodes[1] *= 0.8; nodes[2] *= 1.3
+        w = dict(nodes=nodes, Q=inputs.taylor_green(nodes), G=None, D=None, params=inputs.tgv_params(Re=100.0), nonlinear=1, cfl=0.5)
+    elif case == "jump":
+        w = parity.build_case("jump_blob", 12, 1)
+    else:
+        w = parity.build_case(case, 12, 1, 2.0 if case == "iso_sup" else None)
+    orc, dts = parity.run_oracle(w, 2)
+    monkeypatch.delenv("CGKS_PIPELINE", raising=False)
+    sweep, _ = parity.run_gpu(w, 2, dts=dts)
+    monkeypatch.setenv("CGKS_PIPELINE", "split")
+    split, _ = parity.run_gpu(w, 2, dts=dts)
+    monkeypatch.delenv("CGKS_PIPELINE", raising=False)
+    e_ab = parity.field_errors(sweep, split, w["nodes"], w["Q"])
+    e_sw = parity.field_errors(sweep, orc, w["nodes"], w["Q"])
+    e_sp = parity.field_errors(split, orc, w["nodes"], w["Q"])
+    print(case, "sweep vs split %.1e, sweep vs oracle %.1e, split vs oracle %.1e" % (max(e_ab.values()), max(e_sw.values()), max(e_sp.values())))
+    assert max(e_ab.values()) <= (1e-10 if case == "jump" else 1e-11), max(e_ab, key=e_ab.get)
+    assert max(e_sw.values()) <= 2 * TOL_1 and max(e_sp.values()) <= 2 * TOL_1
+
+
+def test_sweep_lines_cut_into_segments():
+    """The sweep kernels cut the j- and k-lines into segments (each starts with one recomputed face); on a mesh with many
+    more cells along j and k than the shortest segment (24) the result must not depend on it: a 8 x 60 x 56 mesh against the
+    oracle, and bit-identical to its own k-slab pipeline (other k-segments, other first faces)."""
+    from paper_2508_08965_b200 import binding
+    shape = (8, 60, 56)
+    nodes = inputs.cartesian_nodes(shape, 0.0, 2.0 * np.pi)
+    w = dict(nodes=nodes, Q=inputs.taylor_green(nodes), G=None, D=None, params=inputs.tgv_params(Re=100.0), nonlinear=1, cfl=0.5)
+    _check(w, 1, TOL_1)
+    full, _ = parity.run_gpu(w, 2)
+    n = shape[0] * shape[1] * shape[2]; plane = shape[0] * shape[1]
+    budget = 3 * 80 * n * 8 + 5 * n * 8 + 37 * n * 8 + 4096 + 30 * 480 * plane * 8
+    s = binding.Solver(w["nodes"], binding.make_params(**w["params"], nonlinear=1), budget_bytes=budget)
+    assert 24 < s.slab_depth() < shape[2]          # two chunks, the first longer than the shortest segment
+    s.close()
+    slab, _ = parity.run_gpu(w, 2, budget_bytes=budget)
+    for a, b in zip(full, slab):
+        assert np.array_equal(a, b)
 
 
 @pytest.mark.parametrize("name,n,k0", [("sine", 16, None), ("iso_sup", 16, 2.0), ("tgv", 16, None),
