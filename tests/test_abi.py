@@ -109,20 +109,21 @@ def test_flux_flop_constant_is_the_oracle_count():
     spec = importlib.util.spec_from_file_location("bench", os.path.join(ROOT, "bench.py"))
     bench = importlib.util.module_from_spec(spec); spec.loader.exec_module(bench)
     assert counts["flux_point"][1] == bench.FLUX_FLOPS_ORACLE
-    assert counts["flux_point"][0] >= counts["flux_point"][1] > 5 * bench.FLUX_FLOPS_STAGE1
+    assert counts["flux_point"][0] >= counts["flux_point"][1] > 5 * bench.SWEEP_FLOPS_STAGE1
     # the non-zero count of one (cell, variable) reconstruction is bounded below by the non-zeros of M and E (FMA = 2)
     assert counts["recon_var"][1] >= 2 * (1008 + 2184)
 
 
 def test_flux_flop_constants_belong_to_the_committed_kernel_source():
     """bench.py's executed-flop constants were counted with ncu on a specific revision of the flux arithmetic
-    (profiles/r02d_kernels_128.md); a change to gks_flux.cuh / fastmath64.cuh / math_gen.cuh without a re-count fails here."""
+    and of the sweep kernel around it (profiles/r02f_kernels_128.md); a change to gks_flux.cuh / fastmath64.cuh / math_gen.cuh /
+    kernels_fused.cuh without a re-count fails here."""
     import hashlib
     import importlib.util
     csrc = os.path.join(ROOT, "paper_2508_08965_b200", "csrc")
     h = hashlib.sha256()
-    for fn in ("gks_flux.cuh", "fastmath64.cuh", "math_gen.cuh"):
+    for fn in ("gks_flux.cuh", "fastmath64.cuh", "math_gen.cuh", "kernels_fused.cuh"):
         h.update(open(os.path.join(csrc, fn), "rb").read())
     spec = importlib.util.spec_from_file_location("bench", os.path.join(ROOT, "bench.py"))
     bench = importlib.util.module_from_spec(spec); spec.loader.exec_module(bench)
-    assert h.hexdigest()[:16] == bench.FLUX_SOURCE_SHA16, "re-count FLUX_FLOPS_STAGE1/2 with ncu and update FLUX_SOURCE_SHA16"
+    assert h.hexdigest()[:16] == bench.FLUX_SOURCE_SHA16, "re-count SWEEP_FLOPS_STAGE1/2 with ncu and update FLUX_SOURCE_SHA16"
