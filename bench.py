@@ -47,7 +47,7 @@ SWEEP_FP64_PIPE_ACTIVE_NCU = (0.570, 0.586)     # sm__pipe_fp64_cycles_active of
 # cell and stage 1: 40 (Q^n) + 2 x 320 read, 3 x 640 written; stage 2: 3 x 320 read, 3 x 320 written; / 12 points.
 # Measured: dram__bytes_read + write per launch / points, same capture.
 SWEEP_BYTES_ALG = (320.0 + (40 + 640 + 1920) / 12.0, 320.0 + (960 + 960) / 12.0)
-SWEEP_TRAFFIC = (557.0, 480.0)
+SWEEP_TRAFFIC = (556.2, 490.9)
 FP64_PEAK_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12      # SMs x FP64 FMA lanes x 2 x max SM clock = 37.2
 
 
@@ -289,9 +289,22 @@ def run_ours(args):
         planes = (nk_own if use_slab else n) + (2 * nchunks if (use_slab or nchunks > 1) else 0)
         recon_bytes = 2 * psteps * 4480.0 * planes * n * n
         hbm_peak = measured_hbm_peak()
-        roof = {"bound": "alu", "kernel": "sweep_kernel", "achieved": ach, "peak": FP64_PEAK_NOMINAL_TFLOPS, "unit": "TFLOP/s",
-                "frac": ach / FP64_PEAK_NOMINAL_TFLOPS,
-                "frac_at_measured_clock": ach / (FP64_PEAK_NOMINAL_TFLOPS * sm_mhz / 1965.0),
+        # which roof binds (north_star: "the slower of bytes at HBM bandwidth and flops at FP64 peak"): the kernel's arithmetic
+        # intensity, executed flops / algorithmic bytes, against the machine balance
+        alg_bytes_launch = 0.5 * sum(SWEEP_BYTES_ALG) * pts_per_launch
+        gbs = alg_bytes_launch / (fms / fnl * 1e-3) / 1e9
+        t_hbm = gbs / hbm_peak[0]; t_alu = ach / FP64_PEAK_NOMINAL_TFLOPS
+        hbm_bound = t_hbm >= t_alu
+        roof = {"bound": "hbm" if hbm_bound else "alu", "kernel": "sweep_kernel",
+                "achieved": gbs if hbm_bound else ach, "peak": hbm_peak[0] if hbm_bound else FP64_PEAK_NOMINAL_TFLOPS,
+                "unit": "GB/s" if hbm_bound else "TFLOP/s", "frac": max(t_hbm, t_alu),
+                "bound_note": "arithmetic intensity %.2f flop/B (executed flops / algorithmic bytes) against a machine balance of %.2f flop/B "
+                              "(%.1f TFLOP/s FP64 / %.1f GB/s HBM, %s): the %s roof is the slower one for this kernel; both fractions are given"
+                              % ((SWEEP_FLOPS_STAGE1 + SWEEP_FLOPS_STAGE2) / sum(SWEEP_BYTES_ALG), FP64_PEAK_NOMINAL_TFLOPS * 1e3 / hbm_peak[0],
+                                 FP64_PEAK_NOMINAL_TFLOPS, hbm_peak[0], hbm_peak[1], "HBM" if hbm_bound else "FP64"),
+                "hbm": {"achieved": gbs, "peak": hbm_peak[0], "unit": "GB/s", "frac": t_hbm, "peak_source": hbm_peak[1]},
+                "alu": {"achieved": ach, "peak": FP64_PEAK_NOMINAL_TFLOPS, "unit": "TFLOP/s", "frac": t_alu,
+                        "frac_at_measured_clock": ach / (FP64_PEAK_NOMINAL_TFLOPS * sm_mhz / 1965.0)},
                 "flops_per_point_executed": [SWEEP_FLOPS_STAGE1, SWEEP_FLOPS_STAGE2],
                 "flops_per_point_oracle_counted": FLUX_FLOPS_ORACLE,
                 "achieved_with_oracle_count": ach * 2.0 * FLUX_FLOPS_ORACLE / (SWEEP_FLOPS_STAGE1 + SWEEP_FLOPS_STAGE2),
@@ -304,17 +317,19 @@ def run_ours(args):
                               "box runs below it under its 1 kW power cap (frac_at_measured_clock uses the sampled clock); the CPU oracle's "
                               "term-by-term evaluation needs 7x the arithmetic, so its count would give a fraction above 1 (DESIGN.md 7.2)",
                 "traffic": 0.5 * sum(SWEEP_TRAFFIC) * pts_per_launch,
-                "algorithmic_bytes": 0.5 * sum(SWEEP_BYTES_ALG) * pts_per_launch,
+                "algorithmic_bytes": alg_bytes_launch,
                 "traffic_note": "bytes per average launch = ncu dram bytes per point (profiles/r02f_kernels_128.md) x points per launch; "
                                 "algorithmic bytes per point %.0f (stage 1) / %.0f (stage 2)" % SWEEP_BYTES_ALG,
-                "hbm_frac_of_this_kernel": (0.5 * sum(SWEEP_BYTES_ALG) * pts_per_launch / (fms / fnl * 1e-3) / 1e9) / hbm_peak[0],
-                "peak_source": "derived: 148 SMs x 64 FP64 FMA lanes x 2 x 1.965 GHz (DESIGN.md section 7); "
+                "peak_source": "HBM: " + hbm_peak[1] + "; FP64: derived, 148 SMs x 64 FP64 FMA lanes x 2 x 1.965 GHz (DESIGN.md section 7), "
                                "MEASURED_PEAKS.json has no FP64 entry",
                 "peak_dfma_microbench": peak_meas, "frac_of_dfma_microbench": (ach / peak_meas) if peak_meas else None,
                 "avg_launch_ms": fms / fnl, "launches": fnl,
                 "share_of_step": fms / (pms if pms > 0 else 1.0),
                 "kernel_ms_per_step": {k: v[0] / psteps for k, v in kms.items()},
                 "profiled_steps": psteps, "profiled_ms_per_step": pms / psteps,
+                "whole_step": {"algorithmic_bytes_per_cell": 2 * 4480.0 + 12.0 * sum(SWEEP_BYTES_ALG),
+                               "hbm_floor_ms": (2 * 4480.0 + 12.0 * sum(SWEEP_BYTES_ALG)) * cells_rank / hbm_peak[0] / 1e6,
+                               "frac_of_hbm_roofline": (2 * 4480.0 + 12.0 * sum(SWEEP_BYTES_ALG)) * cells_rank / hbm_peak[0] / 1e6 / (pms / psteps)},
                 "other_kernels": {"recon_kernel": {
                     "bound": "hbm", "achieved": recon_bytes / (rms * 1e-3) / 1e9 if rms > 0 else None, "peak": hbm_peak[0], "unit": "GB/s",
                     "frac": (recon_bytes / (rms * 1e-3) / 1e9 / hbm_peak[0]) if rms > 0 else None, "peak_source": hbm_peak[1],
