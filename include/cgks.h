@@ -54,8 +54,8 @@ typedef struct {
   int    geno_r;              /* r = 2; only r = 2 is implemented                               */
 } cgks_params;
 
-/* Bytes of device workspace for a mesh of ni x nj x nk cells (state, stage buffers, metrics, and the slab buffers
-   of reconstructed face values and face fluxes).  `budget_bytes` = 0 asks for the default (largest useful slab up
+/* Bytes of device workspace for a mesh of ni x nj x nk cells (state, stage buffers, metrics, and the slab buffer of
+   reconstructed face values; when the whole mesh fits, also the face-flux buffer the test tap cgks_debug_stage needs).  `budget_bytes` = 0 asks for the default (largest useful slab up
    to ~48 GB of slab buffers); otherwise the slab depth is reduced so that the total stays below the budget, and
    CGKS_ENOMEM is returned when not even a slab of two k-planes fits under it.  (`budget_bytes` is an addition to
    the call list of SURVEY.md 8(b): the 384^3 case needs the caller to say how much of the device it may take.) */
@@ -77,7 +77,11 @@ int cgks_get_state(cgks_ctx*, double* d_Q, double* d_G, double* d_D);
    DESIGN.md reading S3).  Synchronises; returns CGKS_ENONPHYSICAL if an earlier stage flagged a bad cell. */
 int cgks_compute_dt(cgks_ctx*, double cfl, double* dt_host);
 
-/* One two-stage fourth-order step of size dt.  Asynchronous. */
+/* One two-stage fourth-order step of size dt.  Asynchronous.
+   Per stage: one reconstruction kernel (Eq. 11-19), then one sweep kernel per face direction that computes the gas-kinetic
+   flux at the face Gauss points (Eq. 1-7) and accumulates Eq. 8-10 and the S2O4 combine into the state buffers.  With
+   CGKS_PIPELINE=split in the environment at cgks_create time the stage instead runs the three-kernel pipeline of the first
+   rounds (flux -> face-flux buffer -> update): same results to round-off, kept for A/B timing. */
 int cgks_step(cgks_ctx*, double dt);
 
 /* One stage of the step (1: state n -> stage state; 2: stage state -> state n+1); cgks_step(dt) is
@@ -140,7 +144,8 @@ int cgks_slab_depth(const cgks_ctx*);
 long cgks_launch_count(const cgks_ctx*);
 
 /* Device-side duration in milliseconds of the kernels of one class accumulated by the last cgks_step when profiling
-   is switched on with cgks_set_profiling(ctx, 1): 0 reconstruction, 1 flux, 2 update, 3 cfl.  Profiling inserts
+   is switched on with cgks_set_profiling(ctx, 1): 0 reconstruction, 1 flux (the sweep kernels: flux + update), 2 update (three-kernel
+   pipeline only), 3 cfl.  Profiling inserts
    CUDA events on the stream and synchronises at the end of the step. */
 int cgks_set_profiling(cgks_ctx*, int on);
 int cgks_kernel_ms(const cgks_ctx*, int which, double* ms, long* launches);
@@ -152,7 +157,8 @@ int cgks_get_chi(cgks_ctx*, double* d_chi);
 /* Test tap: runs the reconstruction (and, if d_fx != NULL, the flux kernels with step size dt, stage 1) on the
    CURRENT state and copies the slab buffers out: d_pv [480][N] (plane (4m+q)*20 + c: c = v value, 5+3v+r physical
    gradient; NO positivity fallback applied), d_fx [360][N] (plane (4ax+q)*30 + c: Fn, Ft, VL, DtL, VR, DtR).
-   Needs the whole mesh resident (CGKS_ENOMEM otherwise).  The state is not modified. */
+   Needs the whole mesh resident and, for d_fx, room for the face-flux buffer in the workspace (CGKS_ENOMEM otherwise); the flux tap
+   runs the gas-kinetic solver through the thread-per-point kernel of the three-kernel pipeline.  The state is not modified. */
 int cgks_debug_stage(cgks_ctx*, double dt, double* d_pv, double* d_fx);
 
 /* Measures the device's FP64 FMA throughput with a register-resident DFMA micro-benchmark (8 independent chains
