@@ -67,6 +67,16 @@ __device__ __forceinline__ void ld4_ro(const double* p, double& a, double& b, do
   asm("ld.global.nc.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(a), "=d"(b), "=d"(c), "=d"(d) : "l"(__cvta_generic_to_global(p)));
 }
 
+// the same with an L2 evict-last policy: records that neighbouring cells will gather again (one plane of output later)
+__device__ __forceinline__ unsigned long long l2_policy_evict_last() {
+  unsigned long long p;
+  asm("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+  return p;
+}
+__device__ __forceinline__ void ld4_ro_keep(const double* p, unsigned long long pol, double& a, double& b, double& c, double& d) {
+  asm("ld.global.nc.L2::cache_hint.v4.f64 {%0, %1, %2, %3}, [%4], %5;" : "=d"(a), "=d"(b), "=d"(c), "=d"(d) : "l"(__cvta_generic_to_global(p)), "l"(pol));
+}
+
 struct CellIdx { int i, j, k; long ij; long c; };
 // thread t over `cnt` planes starting at plane kA (wrapped).  32-bit index arithmetic: cgks_create rejects meshes with
 // 2^31 cells or more (far beyond 180 GB of state), and 64-bit integer division costs ~100 instructions on the SM.

@@ -46,11 +46,12 @@ template <int AX> __device__ __forceinline__ void eval_axis(const double* a, dou
 template <bool CART>
 struct ReconCell {
   const Mesh& m; const double* qg;      // records { Q, G (3) } of this variable, [n][4]
+  unsigned long long pol;               // L2 policy of the gathers
   double J[9];
   // average difference and (grad Q)' = J0^T grad Q of neighbour cn with the TARGET cell's J0: one 256-bit load
   __device__ __forceinline__ void neighbour(long cn, double q0, double& dq, double* gr) const {
     double q, g0, g1, g2;
-    ld4_ro(qg + 4 * cn, q, g0, g1, g2);
+    ld4_ro_keep(qg + 4 * cn, pol, q, g0, g1, g2);
     dq = q - q0;
     if (CART) { gr[0] = m.h[0] * g0; gr[1] = m.h[1] * g1; gr[2] = m.h[2] * g2; }
     else {
@@ -108,7 +109,7 @@ __global__ void __launch_bounds__(128, 3) recon_kernel(Mesh m, Slab sl, const do
   const int ii[3] = { wrap(x.i - 1, m.ni), x.i, wrap(x.i + 1, m.ni) };
   const int jj[3] = { wrap(x.j - 1, m.nj), x.j, wrap(x.j + 1, m.nj) };
   const int kk[3] = { wrap(x.k - 1, m.nk), x.k, wrap(x.k + 1, m.nk) };
-  ReconCell<CART> rc{ m, W + iQG(v, 0, n), {} };
+  ReconCell<CART> rc{ m, W + iQG(v, 0, n), l2_policy_evict_last(), {} };
   if (!CART) {
 #pragma unroll
     for (int q = 0; q < 9; q++) rc.J[q] = m.met[(MET_J0 + q) * n + x.c];
