@@ -65,6 +65,39 @@ __device__ __forceinline__ double dexp(double x) {
   return (p * s1) * s2;
 }
 
+// log(x) for positive, finite, normal x: x = m 2^e with m in [1/sqrt 2, sqrt 2), log m = 2 atanh(f), f = (m-1)/(m+1),
+// |f| <= 0.1716, odd series up to f^23 (next term < 6e-19); e ln 2 with ln 2 split in two.  Used for the viscosity power
+// law (T/T_ref)^omega = exp(omega log(T/T_ref)); CUDA's log carries slow-path branches (see the header of this file).
+__device__ __forceinline__ double dlog(double x) {
+  int hi = __double2hiint(x);
+  const int lo = __double2loint(x);
+  int e = (hi >> 20) - 1023;
+  hi = (hi & 0x000fffff) | 0x3ff00000;
+  double m = __hiloint2double(hi, lo);                     // [1, 2)
+  const bool big = m > 1.4142135623730951;
+  m = big ? 0.5 * m : m;
+  e += big ? 1 : 0;
+  const double f = (m - 1.0) * drcp(m + 1.0), f2 = f * f;
+  // two interleaved Horner chains in f^4 for sum_{k>=1} f2^k/(2k+1), k = 1..11
+  const double f4 = f2 * f2;
+  double pa = 1.0 / 23.0;                                  // k = 11, 9, 7, 5, 3, 1
+  pa = fma(pa, f4, 1.0 / 19.0);
+  pa = fma(pa, f4, 1.0 / 15.0);
+  pa = fma(pa, f4, 1.0 / 11.0);
+  pa = fma(pa, f4, 1.0 / 7.0);
+  pa = fma(pa, f4, 1.0 / 3.0);
+  double pb = 1.0 / 21.0;                                  // k = 10, 8, 6, 4, 2
+  pb = fma(pb, f4, 1.0 / 17.0);
+  pb = fma(pb, f4, 1.0 / 13.0);
+  pb = fma(pb, f4, 1.0 / 9.0);
+  pb = fma(pb, f4, 1.0 / 5.0);
+  const double p = f2 * fma(pb, f2, pa);                   // sum_{k>=1} f2^k/(2k+1)
+  const double tf = 2.0 * f;
+  const double lm = fma(tf, p, tf);
+  const double de = (double)e;
+  return fma(de, 6.93147180369123816490e-01, fma(de, 1.90821492927058770002e-10, lm));
+}
+
 // erfc(|x|) * exp(x^2) * (1 + 2|x|) as a polynomial in t = (|x|-4)/(|x|+4): even/odd split, two Horner chains
 __device__ __forceinline__ double erfcx_poly(double t) {
   const double CGKS_ERFCX_P[CGKS_ERFCX_NP] = { CGKS_ERFCX_P_LIST };

@@ -298,7 +298,7 @@ __device__ __forceinline__ void gks_flux_local(const GasConst& gc, double dt, do
   double tau_phys = 0.0;
   if (gc.mu_ref > 0.0) {
     double visc = gc.mu_ref;
-    if (gc.omega != 0.0) visc *= dexp(gc.omega * log(g0.hil * gc.inv_T_ref));      // (T/T_ref)^omega, T = p/rho
+    if (gc.omega != 0.0) visc *= dexp(gc.omega * dlog(g0.hil * gc.inv_T_ref));      // (T/T_ref)^omega, T = p/rho
     tau_phys = visc * (2.0 * g0.lam * g0.irho);                                    // mu / p0
   }
   const double dpr = ddiv(fabs(pl - pr), fabs(pl + pr));

@@ -309,9 +309,24 @@ __global__ void __launch_bounds__(SW_TPB, FLUX_MINB) sweep_kernel(Mesh m, Slab s
         double d0 = 0;
         if (!STAGE2) d0 = P[2][v] - M[2][v];
         if (CART) {
-          sFt = qsum(P[1][v] - M[1][v]);
-          sD[0] = qsum(d1);
-          if (!STAGE2) { sF = qsum(P[0][v] - M[0][v]); sV[0] = qsum(d0); }
+          // Only lane 0 of the quad needs the flux sums (its component is Q) and only lane 1 + AXIS the sums of the interface
+          // values (its component is G_AXIS): a reduce-scatter.  Each lane keeps one of the two kinds and hands the other to
+          // its xor-1 partner, then the two lanes that keep the same kind add up: half the shuffles of four full butterflies,
+          // and the same order of additions, (q0 + q1) + (q2 + q3), in the lane that uses the sum.
+          const bool keepF = (AXIS == 1) ? (q == 0 || q == 3) : ((q & 1) == 0);
+          constexpr int PAIR = (AXIS == 1) ? 3 : 2;
+          const double fT = P[1][v] - M[1][v];
+          double kT = keepF ? fT : d1;
+          kT += __shfl_xor_sync(0xffffffffu, keepF ? d1 : fT, 1);
+          kT += __shfl_xor_sync(0xffffffffu, kT, PAIR);
+          sFt = kT; sD[0] = kT;
+          if (!STAGE2) {
+            const double fN = P[0][v] - M[0][v];
+            double kN = keepF ? fN : d0;
+            kN += __shfl_xor_sync(0xffffffffu, keepF ? d0 : fN, 1);
+            kN += __shfl_xor_sync(0xffffffffu, kN, PAIR);
+            sF = kN; sV[0] = kN;
+          }
         } else {
           sFt = qsum(P[1][v] * Sp - M[1][v] * Sm);
 #pragma unroll

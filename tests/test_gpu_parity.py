@@ -310,10 +310,17 @@ def test_special_functions_of_the_flux_kernel():
     import mpmath as mp
     from scipy import special
     from paper_2508_08965_b200 import binding
+    mp.mp.dps = 40
     rng = np.random.default_rng(7)
     x = np.concatenate([10.0 ** rng.uniform(-12, 12, 20000), rng.uniform(0.5, 2.0, 20000)])
     np.testing.assert_allclose(binding.debug_math(0, x), 1.0 / x, rtol=4e-16)
     np.testing.assert_allclose(binding.debug_math(1, x), 1.0 / np.sqrt(x), rtol=6e-16)
+    xl = np.concatenate([x, rng.uniform(0.99, 1.01, 20000), [1.0, 2.0 ** 0.5, 0.5 ** 0.5, 1.4142135623730951, 1.4142135623730954]])
+    gl = binding.debug_math(5, xl)
+    for a, b in zip(xl[::97], gl[::97]):         # the power law of the viscosity: log against mpmath, absolute 2e-16 near 1
+        r = mp.log(mp.mpf(float(a)))
+        assert abs(mp.mpf(float(b)) - r) <= 3e-16 * max(abs(r), mp.mpf(1) / 8), a
+    np.testing.assert_allclose(gl, np.log(xl), rtol=1e-15, atol=3e-17)
     xe = np.concatenate([rng.uniform(-700, 10, 20000), rng.uniform(-1, 1, 20000)])
     np.testing.assert_allclose(binding.debug_math(2, xe), np.exp(xe), rtol=1e-15)
     xu = np.array([-745.0, -760.0, -800.0, -1e5, -1e300])
