@@ -12,8 +12,9 @@
  * Parity status of the individual functions (see DESIGN.md section 4 for the pins):
  *   reconstruction matrix, evaluation, S2O4 combine, GKS moments/flux ... pinned
  *   GENO path function reading G2/G3 ................ pinned only via Tables 1-2 (pattern)
- *   l/r interface-value blend F3, Prandtl fix F2, dt formula S3, positivity R9,
- *   bootstrap S2 ...................................... parity unpinned (paper silent)
+ *   Prandtl fix F2, dt formula S3, positivity R9, bootstrap S2, the one-sided parts
+ *   and the weight of the interface blend F3 ......... arithmetic pinned (tests/test_oracle_pins2.py);
+ *                                                      the CHOICE of these readings: parity unpinned (paper silent)
  *
  * All pointers are HOST pointers.  Arrays are structure-of-arrays, i fastest:
  *   nodes [3][nk+1][nj+1][ni+1], Q [5][nk][nj][ni], G [5][3][nk][nj][ni],

@@ -292,3 +292,76 @@ def test_geno_formulas_on_worked_examples():
         alpha = 2.0 * ah / (ah + al)
         assert abs(chi - math.tanh(5.0 * alpha) / math.tanh(5.0)) < 1e-11, (a_, c_, chi)
     assert chi > 0.999                                                       # nearly linear data: the quartic is kept
+
+
+# ----------------------------------------------------------------------------- reading F3: the one-sided ingredients
+def _euler_flux(W, d):
+    rho = W[0]; U = W[1:4] / rho
+    p = (GAMMA - 1.0) * (W[4] - 0.5 * rho * U @ U)
+    F = W * U[d]
+    F[1 + d] += p; F[4] += p * U[d]
+    return F
+
+
+def test_F3_one_sided_part_is_the_euler_time_derivative():
+    """Reading F3: the interface values handed to the two cells are V^s = (1-w) Q^e + w W^s and
+    Q_t^s = (1-w) Q_t^e + w int psi A^s g_s, w = exp(-dt/tau0), tau0 = c2 |pl-pr|/|pl+pr| dt, with ONE equilibrium part Q^e,
+    Q_t^e for both sides.  Hence V^l - V^r = w (W^l - W^r) and Q_t^l - Q_t^r = w (dW^l/dt - dW^r/dt), where the compatibility
+    condition makes the one-sided time derivative the Euler equations applied to the one-sided polynomial,
+    dW/dt = - sum_d dF_d(W)/dx_d: written here from the textbook Euler flux (central differences of F_d along the slope, no
+    kinetic arithmetic).  Pins sign, frame rotation and the slope -> time-slope solve of the one-sided part, and the weight.
+    (The sum of the two sides contains Q^e, which P7b pins by brute force; the limit w -> 1 does not isolate the one-sided
+    part: (1-w) Q^e tends to dt times a slope term, because Q^e grows like tau.)"""
+    rng = np.random.default_rng(11)
+    from tests.test_oracle_gks import random_frame
+
+    def euler_dt(W, g):
+        eps = 1e-6
+        r = np.zeros(5)
+        for d in range(3):
+            r -= (_euler_flux(W + eps * g[:, d], d) - _euler_flux(W - eps * g[:, d], d)) / (2 * eps)
+        return r
+    for c2 in (5.0, 0.8, 60.0):
+        n, t1 = random_frame(rng)
+        WL = cons(1.0, [0.35, -0.2, 0.1], 1.0); WR = cons(0.5, [0.15, 0.1, -0.05], 0.3)
+        gL = 0.3 * rng.standard_normal((5, 3)); gR = 0.3 * rng.standard_normal((5, 3))
+        eL, eR = euler_dt(WL, gL), euler_dt(WR, gR)
+        out = ref.flux_point(ref.make_params(gamma=GAMMA, Pr=1.0, mu_ref=0.0, tau_c1=0.05, tau_c2=c2), 0.01, WL, gL, WR, gR, n, t1)
+        w = math.exp(-1.0 / (c2 * abs(1.0 - 0.3) / (1.0 + 0.3)))
+        np.testing.assert_allclose(out[2] - out[4], w * (WL - WR), rtol=1e-10, atol=1e-11)
+        np.testing.assert_allclose(out[3] - out[5], w * (eL - eR), rtol=1e-7, atol=1e-8)
+        assert np.abs(eL - eR).max() > 1e-2 and w > 0.09          # the two sides really differ, the weight is not ~0
+
+
+# ----------------------------------------------------------------------------- reading S2: bootstrap of G and D
+def test_S2_bootstrap_symbol_on_the_sheared_mesh():
+    """Reading S2 (the paper is silent on the initial derivative dof): G and D from the fourth-order central difference
+    (8 (Q+1 - Q-1) - (Q+2 - Q-2))/12 of the cell averages along each index direction, G = J0^-T of that reference-space
+    vector, the four line differences of an axis = its component.  For a plane wave in the lattice
+    coordinates, Q = 2 + sin(a . xi), the difference quotient of the cell averages has the closed form
+    A cos(a . xi_c) (8 sin(a_r h) - sin(2 a_r h))/6 with A the product of the three sinc factors of the cell average: pins
+    the stencil weights, their sign, the axis -> line-difference placement and, on the non-symmetric affine mesh, J0^-T
+    against a transposed or missing transform."""
+    n = 12; h = 2.0 * math.pi / n
+    nodes = inputs.sheared_nodes(n, h)
+    a = np.array([1.0, 2.0, -1.0])
+    k, j, i = np.meshgrid(np.arange(n) + 0.5, np.arange(n) + 0.5, np.arange(n) + 0.5, indexing="ij")
+    phase = a[0] * i * h + a[1] * j * h + a[2] * k * h
+    amp = np.prod([math.sin(0.5 * ar * h) / (0.5 * ar * h) for ar in a])
+    Q = np.zeros((5, n, n, n))
+    Q[0] = 2.0 + amp * np.sin(phase)
+    Q[1] = 0.3 * Q[0]; Q[2] = -0.1 * Q[0]; Q[3] = 0.2 * Q[0]; Q[4] = 3.0 + 0.5 * amp * np.cos(phase)
+    s = ref.RefSolver(nodes, ref.make_params()); s.set_state(Q)
+    _, Gb, Db = s.get_state(); s.close()
+    sym = np.array([(8.0 * math.sin(ar * h) - math.sin(2.0 * ar * h)) / 6.0 for ar in a])
+    J0 = inputs.SHEAR * h                                  # columns = N2-N1, N3-N1, N4-N1 (reading R1)
+    for v, (c_sin, c_cos) in enumerate([(1.0, 0.0), (0.3, 0.0), (-0.1, 0.0), (0.2, 0.0), (0.0, 0.5)]):
+        dphase = amp * (c_sin * np.cos(phase) - c_cos * np.sin(phase))          # d/d(phase) of variable v's wave
+        dref = sym[:, None, None, None] * dphase[None]                         # reference-space derivative per index direction
+        Gexp = np.einsum("rs,skji->rkji", np.linalg.inv(J0).T, dref)
+        np.testing.assert_allclose(Gb[v], Gexp, atol=2e-13)
+        for r in range(3):
+            for q in range(4):
+                np.testing.assert_allclose(Db[v, 4 * r + q], dref[r], atol=2e-13)
+    # negative control: the transposed transform differs by far more than the tolerance
+    assert np.abs(np.einsum("rs,skji->rkji", np.linalg.inv(J0), dref) - Gexp).max() > 1e-2
