@@ -247,7 +247,7 @@ def run_ours(args):
             def e2e_step():
                 solver.set_state(Qhost.to(dev, non_blocking=True))
                 step(compute_dt(0.5))
-                Qout.copy_(solver.get_state()[0], non_blocking=True)
+                Qout.copy_(solver.get_state(derivatives=False)[0], non_blocking=True)
                 torch.cuda.synchronize(dev)
         else:
             def e2e_step():

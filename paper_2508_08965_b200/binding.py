@@ -174,11 +174,13 @@ class Solver:
         self._check(lib().cgks_set_state(self._h, _ptr(Q), _ptr(G), _ptr(D)))
         torch.cuda.current_stream(self.device).synchronize()      # the inputs may be temporaries
 
-    def get_state(self):
+    def get_state(self, derivatives=True):
+        """(Q, G, D) of the current state; derivatives=False returns (Q, None, None) without allocating the 75 derivative
+        fields (cgks_get_state takes NULL for what is not wanted)."""
         s = (self.nk, self.nj, self.ni)
         Q = torch.empty((5,) + s, dtype=torch.float64, device=self.device)
-        G = torch.empty((5, 3) + s, dtype=torch.float64, device=self.device)
-        D = torch.empty((5, 12) + s, dtype=torch.float64, device=self.device)
+        G = torch.empty((5, 3) + s, dtype=torch.float64, device=self.device) if derivatives else None
+        D = torch.empty((5, 12) + s, dtype=torch.float64, device=self.device) if derivatives else None
         self._check(lib().cgks_get_state(self._h, _ptr(Q), _ptr(G), _ptr(D)))
         return Q, G, D
 
