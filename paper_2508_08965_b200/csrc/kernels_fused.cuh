@@ -26,9 +26,12 @@ namespace cgks {
 constexpr int SW_TPB = 128;                  // 4 warps; FLUX_MINB blocks per SM (254 registers per thread)
 constexpr int SW_CELLS = 8;                  // cells per warp tile
 constexpr int SW_SMEM_IN = 40 * SW_TPB;      // doubles: staged inputs [20 chunks][SW_TPB][2]
-constexpr int SW_SMEM_X = 20 * SW_TPB;       // doubles: hand-over values [20][SW_TPB]
 constexpr int SW_SMEM_RMW = 2 * 10 * SW_TPB; // doubles: read-modify-write operands [2 (step parity)][10][SW_TPB]
-constexpr int SW_SMEM_BYTES = (SW_SMEM_IN + SW_SMEM_X + SW_SMEM_RMW) * 8;
+// doubles: hand-over values [20 (+ 4 on general meshes: vector area and area of the face)][SW_TPB]
+__host__ __device__ constexpr int sw_smem_x(bool cart) { return (cart ? 20 : 24) * SW_TPB; }
+// doubles, general meshes only: [2 (step parity)] + face vector area (3), tangent (3), cell volume
+__host__ __device__ constexpr int sw_smem_met(bool cart) { return cart ? 0 : 2 * 7 * SW_TPB; }
+__host__ __device__ constexpr int sw_smem_bytes(bool cart) { return (SW_SMEM_IN + sw_smem_x(cart) + SW_SMEM_RMW + sw_smem_met(cart)) * 8; }
 
 struct SweepPrm {
   int kA, cnt;       // planes kA .. kA+cnt-1 (wrapped) are updated
@@ -102,7 +105,8 @@ __global__ void __launch_bounds__(SW_TPB, FLUX_MINB) sweep_kernel(Mesh m, Slab s
   extern __shared__ __align__(16) double sm[];
   double* smf = sm;                                      // staged inputs
   double* smx = sm + SW_SMEM_IN;                         // hand-over values
-  double* smr = sm + SW_SMEM_IN + SW_SMEM_X;             // read-modify-write operands
+  double* smr = sm + SW_SMEM_IN + sw_smem_x(CART);       // read-modify-write operands
+  double* smm = sm + SW_SMEM_IN + sw_smem_x(CART) + SW_SMEM_RMW;      // face metrics of the step (general meshes)
   const int tid = threadIdx.x, lane = tid & 31, q = lane & 3, cl = lane >> 2;
   const int gw = blockIdx.x * (SW_TPB / 32) + (tid >> 5), nw = gridDim.x * (SW_TPB / 32);
   const long n = m.n;
@@ -117,6 +121,15 @@ __global__ void __launch_bounds__(SW_TPB, FLUX_MINB) sweep_kernel(Mesh m, Slab s
       for (int c = 0; c < 10; c++) cp_async16(dst + c * (2 * SW_TPB), pL + (long)(c >> 1) * (4 * sl.stride_pv) + 2 * (c & 1));
 #pragma unroll
       for (int c = 0; c < 10; c++) cp_async16(dst + (10 + c) * (2 * SW_TPB), pR + (long)(c >> 1) * (4 * sl.stride_pv) + 2 * (c & 1));
+      if (!CART) {
+        double* mt = smm + par * (7 * SW_TPB) + tid;
+#pragma unroll
+        for (int r = 0; r < 3; r++) {
+          cp_async8(mt + r * SW_TPB, m.met + (MET_AREA + 3 * AXIS + r) * n + p.cL);
+          cp_async8(mt + (3 + r) * SW_TPB, m.met + (MET_TAN + 3 * AXIS + r) * n + p.cL);
+        }
+        cp_async8(mt + 6 * SW_TPB, m.met + MET_VOL * n + p.cL);
+      }
       if (s >= 0) {
         double* r = smr + par * (10 * SW_TPB) + tid;
         const long oq = 4 * (long)p.cL + q, sq = 4 * n;
@@ -155,6 +168,20 @@ __global__ void __launch_bounds__(SW_TPB, FLUX_MINB) sweep_kernel(Mesh m, Slab s
       WLg[v] = l0.x; gL[3 * v] = l0.y; gL[3 * v + 1] = l1.x; gL[3 * v + 2] = l1.y;
       WRg[v] = r0.x; gR[3 * v] = r0.y; gR[3 * v + 1] = r1.x; gR[3 * v + 2] = r1.y;
     }
+    // general meshes: this face's frame (n, t1, t2), vector area A and area S from the staged metrics; built twice per step (before
+    // and after the solver) instead of being carried through it in 26 registers
+    auto face_frame = [&](double (*f)[3], double* A, double& S) {
+      const double* mt = smm + par * (7 * SW_TPB) + tid;
+#pragma unroll
+      for (int r = 0; r < 3; r++) { A[r] = mt[r * SW_TPB]; f[1][r] = mt[(3 + r) * SW_TPB]; }
+      const double AA = A[0] * A[0] + A[1] * A[1] + A[2] * A[2], iS = drsqrt(AA);     // branch-free; stale but finite on lanes without a cell
+      S = AA * iS;
+#pragma unroll
+      for (int r = 0; r < 3; r++) f[0][r] = A[r] * iS;
+      f[2][0] = f[0][1] * f[1][2] - f[0][2] * f[1][1];
+      f[2][1] = f[0][2] * f[1][0] - f[0][0] * f[1][2];
+      f[2][2] = f[0][0] * f[1][1] - f[0][1] * f[1][0];
+    };
     // the step after this one (warp-uniform): its inputs stream in during the arithmetic of this one
     int nline = line, ns = s + 1;
     if (ns >= L.len) { nline = line + nw; ns = -1; if (nline < sp.nlines) L = sweep_line<AXIS>(m, sp, nline, cl); }
@@ -167,7 +194,7 @@ __global__ void __launch_bounds__(SW_TPB, FLUX_MINB) sweep_kernel(Mesh m, Slab s
     const bool act = cur.act;
     double P[4][5];       // this face, global frame: F^n, F_t^n, own-side (left) value and time derivative
     double R[2][5];       // right-hand interface value and time derivative: they belong to the next cell
-    double fr[3][3];
+    double A[3] = { 0, 0, 0 }, Sface = 0.0;      // general meshes: vector area and area of this face
     {
       // positivity (reading R9, point-wise): a non-physical reconstructed state falls back to the cell average
       if (act && !admissible(WLg)) {
@@ -196,16 +223,8 @@ __global__ void __launch_bounds__(SW_TPB, FLUX_MINB) sweep_kernel(Mesh m, Slab s
           for (int a = 0; a < 3; a++) { SL[dd][1 + a] = gL[3 * (1 + pm[a]) + pm[dd]]; SR[dd][1 + a] = gR[3 * (1 + pm[a]) + pm[dd]]; }
         }
       } else {
-        double A[3];
-        const long cg = act ? cur.cL : 0;
-#pragma unroll
-        for (int r = 0; r < 3; r++) { A[r] = m.met[(MET_AREA + 3 * AXIS + r) * n + cg]; fr[1][r] = m.met[(MET_TAN + 3 * AXIS + r) * n + cg]; }
-        const double S = sqrt(A[0] * A[0] + A[1] * A[1] + A[2] * A[2]);
-#pragma unroll
-        for (int r = 0; r < 3; r++) fr[0][r] = A[r] / S;
-        fr[2][0] = fr[0][1] * fr[1][2] - fr[0][2] * fr[1][1];
-        fr[2][1] = fr[0][2] * fr[1][0] - fr[0][0] * fr[1][2];
-        fr[2][2] = fr[0][0] * fr[1][1] - fr[0][1] * fr[1][0];
+        double fr[3][3], A0[3], S0;
+        face_frame(fr, A0, S0);
 #pragma unroll
         for (int side = 0; side < 2; side++) {
           const double* Wg = side ? WRg : WLg; const double* gg = side ? gR : gL;
@@ -227,6 +246,8 @@ __global__ void __launch_bounds__(SW_TPB, FLUX_MINB) sweep_kernel(Mesh m, Slab s
       double out[6][5];      // Fn, Ft, VL, DL, VR, DR in the face frame
       gks_flux_local<STAGE2>(gc, dt, idt, WL, SL, WR, SR, out[0], out[1], out[2], out[3], out[4], out[5]);
       // back to the global frame
+      double fr[3][3];
+      if (!CART) face_frame(fr, A, Sface);
 #pragma unroll
       for (int g = 0; g < 6; g++) {
         if (STAGE2 && (g == 0 || g == 2 || g == 4)) continue;
@@ -244,9 +265,15 @@ __global__ void __launch_bounds__(SW_TPB, FLUX_MINB) sweep_kernel(Mesh m, Slab s
     }
     // ---- hand-over: M = what the face below this cell left (F^n, F_t^n, right-hand value and time derivative)
     double M[4][5];
+    double Am[3] = { 0, 0, 0 }, Sm = 0;      // general meshes: vector area and area of the - face (the + face of the cell below)
     {
       double* xs = smx + tid;
       auto put = [&]() {
+        if (!CART) {
+#pragma unroll
+          for (int r = 0; r < 3; r++) xs[(20 + r) * SW_TPB] = A[r];
+          xs[23 * SW_TPB] = Sface;
+        }
         if (!STAGE2) {
 #pragma unroll
           for (int v = 0; v < 5; v++) { xs[v * SW_TPB] = P[0][v]; xs[(5 + v) * SW_TPB] = P[1][v]; xs[(10 + v) * SW_TPB] = R[0][v]; xs[(15 + v) * SW_TPB] = R[1][v]; }
@@ -256,6 +283,11 @@ __global__ void __launch_bounds__(SW_TPB, FLUX_MINB) sweep_kernel(Mesh m, Slab s
         }
       };
       auto get = [&](const double* src) {
+        if (!CART) {
+#pragma unroll
+          for (int r = 0; r < 3; r++) Am[r] = src[(20 + r) * SW_TPB];
+          Sm = src[23 * SW_TPB];
+        }
         if (!STAGE2) {
 #pragma unroll
           for (int v = 0; v < 5; v++) { M[0][v] = src[v * SW_TPB]; M[1][v] = src[(5 + v) * SW_TPB]; M[2][v] = src[(10 + v) * SW_TPB]; M[3][v] = src[(15 + v) * SW_TPB]; }
@@ -279,21 +311,9 @@ __global__ void __launch_bounds__(SW_TPB, FLUX_MINB) sweep_kernel(Mesh m, Slab s
     (void)NX;
     if (s >= 0) {
       // ---- Eq. 8-10 restricted to the two faces of this direction, S2O4 combine
-      double Ap[3] = { 0, 0, 0 }, Am[3] = { 0, 0, 0 }, Sp = 0, Sm = 0, cf;
-      if (CART) cf = 0.25 / m.h[AXIS];
-      else {
-        const int cg = act ? cur.cL : 0;
-        // the cell below along AXIS owns the - face
-        int cm;
-        if (AXIS == 0) { const int i = cg % m.ni; cm = (i == 0) ? cg + m.ni - 1 : cg - 1; }
-        else if (AXIS == 1) { const int ij = cg % (int)m.plane; cm = (ij < m.ni) ? cg + (int)m.plane - m.ni : cg - m.ni; }
-        else { cm = (cg < (int)m.plane) ? cg + (int)(n - m.plane) : cg - (int)m.plane; }
-#pragma unroll
-        for (int r = 0; r < 3; r++) { Ap[r] = m.met[(MET_AREA + 3 * AXIS + r) * n + cg]; Am[r] = m.met[(MET_AREA + 3 * AXIS + r) * n + cm]; }
-        Sp = sqrt(Ap[0] * Ap[0] + Ap[1] * Ap[1] + Ap[2] * Ap[2]); Sm = sqrt(Am[0] * Am[0] + Am[1] * Am[1] + Am[2] * Am[2]);
-        cf = 0.25 / m.met[MET_VOL * n + cg];
-      }
-      auto qsum = [&](double x) { x += __shfl_xor_sync(0xffffffffu, x, 1); x += __shfl_xor_sync(0xffffffffu, x, 2); return x; };
+      double cf;
+      const double* Ap = A; const double Sp = Sface;
+      if (CART) cf = 0.25 / m.h[AXIS]; else cf = 0.25 * drcp(smm[par * (7 * SW_TPB) + 6 * SW_TPB + tid]);      // 1/(4 |Omega|)
       const double hdt = 0.5 * dt;
       const double* rb = smr + par * (10 * SW_TPB) + tid;
       const int comp = q - 1;      // gradient component owned by this lane (q = 0: the cell average)
@@ -328,14 +348,30 @@ __global__ void __launch_bounds__(SW_TPB, FLUX_MINB) sweep_kernel(Mesh m, Slab s
             sF = kN; sV[0] = kN;
           }
         } else {
-          sFt = qsum(P[1][v] * Sp - M[1][v] * Sm);
+          // General meshes: lane 0 needs the two flux sums, lane 1 + r the sums of (interface value) x (component r of the
+          // vector areas): four kinds, one per lane.  Reduce-scatter in two rounds: the halves of the quad exchange the two
+          // kinds that belong to the other half (xor 2), then the partners exchange the other's kind (xor 1).
+          double kT[4], kN[4];
+          kT[0] = P[1][v] * Sp - M[1][v] * Sm;
 #pragma unroll
-          for (int r = 0; r < 3; r++) sD[r] = qsum(P[3][v] * Ap[r] - M[3][v] * Am[r]);
+          for (int r = 0; r < 3; r++) kT[1 + r] = P[3][v] * Ap[r] - M[3][v] * Am[r];
           if (!STAGE2) {
-            sF = qsum(P[0][v] * Sp - M[0][v] * Sm);
+            kN[0] = P[0][v] * Sp - M[0][v] * Sm;
 #pragma unroll
-            for (int r = 0; r < 3; r++) sV[r] = qsum(P[2][v] * Ap[r] - M[2][v] * Am[r]);
+            for (int r = 0; r < 3; r++) kN[1 + r] = P[2][v] * Ap[r] - M[2][v] * Am[r];
           }
+          const bool hi = (q & 2) != 0, odd = (q & 1) != 0;
+          auto rs = [&](const double* k) {
+            double a = hi ? k[2] : k[0], b = hi ? k[3] : k[1];            // kinds of my half
+            a += __shfl_xor_sync(0xffffffffu, hi ? k[0] : k[2], 2);
+            b += __shfl_xor_sync(0xffffffffu, hi ? k[1] : k[3], 2);
+            double mine = odd ? b : a;
+            mine += __shfl_xor_sync(0xffffffffu, odd ? a : b, 1);
+            return mine;                                                  // kind q, summed over the quad
+          };
+          const double tT = rs(kT);
+          sFt = tT; sD[0] = tT; sD[1] = tT; sD[2] = tT;
+          if (!STAGE2) { const double tN = rs(kN); sF = tN; sV[0] = tN; sV[1] = tN; sV[2] = tN; }
         }
         // this lane's component of the record { Q, G_x, G_y, G_z }
         double gV = 0.0, gD = 0.0;      // gradient sums of the values / of the time derivatives, this lane's component
