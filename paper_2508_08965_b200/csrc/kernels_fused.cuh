@@ -18,6 +18,7 @@
 // 2, which updates the saved buffer in place) read-modify-write them; these operands are prefetched with cp.async together
 // with the 2 x 20 reconstructed inputs of the next step, one step ahead of the arithmetic.  No block-level synchronisation,
 // no atomics: the order of every floating-point sum is fixed, results are deterministic and independent of the slab depth.
+// General meshes: the face frame comes from metrics staged the same way, the - face's vector area travels with the hand-over.
 #pragma once
 #include "kernels_stage.cuh"
 
@@ -101,7 +102,6 @@ __global__ void __launch_bounds__(SW_TPB, FLUX_MINB) sweep_kernel(Mesh m, Slab s
                                                                   double* Wsave, GasConst gc, double dt, double idt) {
   constexpr bool STAGE2 = (STAGE == 2);
   constexpr bool FIRST = (STAGE == 1 && AXIS == 0);      // writes the records instead of accumulating into them
-  constexpr int NX = STAGE2 ? 10 : 20;                   // numbers handed to the next cell per point
   extern __shared__ __align__(16) double sm[];
   double* smf = sm;                                      // staged inputs
   double* smx = sm + SW_SMEM_IN;                         // hand-over values
@@ -308,7 +308,6 @@ __global__ void __launch_bounds__(SW_TPB, FLUX_MINB) sweep_kernel(Mesh m, Slab s
         if (act) put();
       }
     }
-    (void)NX;
     if (s >= 0) {
       // ---- Eq. 8-10 restricted to the two faces of this direction, S2O4 combine
       double cf;
