@@ -98,6 +98,12 @@ __device__ __forceinline__ double dlog(double x) {
   return fma(de, 6.93147180369123816490e-01, fma(de, 1.90821492927058770002e-10, lm));
 }
 
+// tanh(x) for x >= 0 (the path function of the GENO blend): (1 - e)/(1 + e), e = exp(-2x); absolute error ~1e-16
+__device__ __forceinline__ double dtanh_pos(double x) {
+  const double e = dexp(-2.0 * x);
+  return (1.0 - e) * drcp(1.0 + e);
+}
+
 // erfc(|x|) * exp(x^2) * (1 + 2|x|) as a polynomial in t = (|x|-4)/(|x|+4): even/odd split, two Horner chains
 __device__ __forceinline__ double erfcx_poly(double t) {
   const double CGKS_ERFCX_P[CGKS_ERFCX_NP] = { CGKS_ERFCX_P_LIST };

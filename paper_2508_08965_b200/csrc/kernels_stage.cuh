@@ -103,8 +103,8 @@ __global__ void __launch_bounds__(128, 3) recon_kernel(Mesh m, Slab sl, const do
   const CellIdx x = cell_of(m, t, kA);
   const long n = m.n;
   if (v == 0) {      // physical admissibility of the incoming cell average (reported by cgks_status / cgks_compute_dt)
-    const double rho = W[iQG(0, x.c, n)], mx = W[iQG(1, x.c, n)], my = W[iQG(2, x.c, n)], mz = W[iQG(3, x.c, n)], E = W[iQG(4, x.c, n)];
-    if (!(rho > 0.0) || !(E - 0.5 * (mx * mx + my * my + mz * mz) / rho > 0.0)) atomicOr(flag, 1);
+    const double w5[5] = { W[iQG(0, x.c, n)], W[iQG(1, x.c, n)], W[iQG(2, x.c, n)], W[iQG(3, x.c, n)], W[iQG(4, x.c, n)] };
+    if (!admissible(w5)) atomicOr(flag, 1);      // rho > 0 and rho E - |m|^2/2 > 0: no division
   }
   const int ii[3] = { wrap(x.i - 1, m.ni), x.i, wrap(x.i + 1, m.ni) };
   const int jj[3] = { wrap(x.j - 1, m.nj), x.j, wrap(x.j + 1, m.nj) };
@@ -140,18 +140,18 @@ __global__ void __launch_bounds__(128, 3) recon_kernel(Mesh m, Slab sl, const do
       b[mm / 2] = (mm % 2 == 0) ? dface[mm] : -dface[mm];
       const double IS = b[0] * b[0] + b[1] * b[1] + b[2] * b[2];
       const double tt = IS + rp.eps, t2 = tt * tt;
-      const double wb = (1.0 / 6.0) / (t2 * t2 * tt);               // d_m/(IS_m + eps)^5
+      const double wb = (1.0 / 6.0) * drcp(t2 * t2 * tt);           // d_m/(IS_m + eps)^5
       wsum += wb; bw[0] += wb * b[0]; bw[1] += wb * b[1]; bw[2] += wb * b[2];
     }
-    // path function (readings G2, G3)
+    // path function (readings G2, G3); divisions and tanh are the branch-free ones of fastmath64.cuh
     const double IS1 = recon_IS1(a), IS2 = recon_IS2(a), ISt = recon_IS34(a);
     const double ISH = IS1 + IS2 + ISt;
-    const double rH = ISt / (ISH + rp.eps), rL = ISt / (IS1 + rp.eps);
+    const double rH = ddiv(ISt, ISH + rp.eps), rL = ddiv(ISt, IS1 + rp.eps);
     const double aH = 1.0 + rH * rH, aL = 1.0 + rL * rL;
-    const double alpha = 2.0 * aH / (aH + aL);
-    chi = tanh(rp.C * alpha) * rp.inv_tanhC;
+    const double alpha = ddiv(2.0 * aH, aH + aL);
+    chi = dtanh_pos(rp.C * alpha) * rp.inv_tanhC;
     // Eq. 16 as one polynomial: chi P4 + (1-chi) sum_m omega_m P1_m
-    const double w1 = (1.0 - chi) / wsum;
+    const double w1 = ddiv(1.0 - chi, wsum);
 #pragma unroll
     for (int b = 0; b < 3; b++) a[b] = chi * a[b] + w1 * bw[b];
 #pragma unroll
@@ -165,7 +165,7 @@ __global__ void __launch_bounds__(128, 3) recon_kernel(Mesh m, Slab sl, const do
 #pragma unroll
     for (int q = 0; q < 9; q++) Ji[q] = m.met[(MET_J0INV + q) * n + x.c];
   }
-  const double ih[3] = { 1.0 / m.h[0], 1.0 / m.h[1], 1.0 / m.h[2] };
+  const double ih[3] = { drcp(m.h[0]), drcp(m.h[1]), drcp(m.h[2]) };
   auto store_axis = [&](int ax, const double* o) {
 #pragma unroll
     for (int l = 0; l < 8; l++) {
