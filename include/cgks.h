@@ -167,7 +167,7 @@ int cgks_debug_stage(cgks_ctx*, double dt, double* d_pv, double* d_fx);
 int cgks_fp64_peak(void* cuda_stream, double* tflops);
 
 /* Test tap for the branch-free fp64 special functions of the flux kernel (csrc/fastmath64.cuh): evaluates function
-   `which` (0: 1/x, 1: 1/sqrt(x), 2: exp(x), 3: erfc(x), 4: exp(-x^2) as returned together with erfc, 5: log(x)) on n device values. */
+   `which` (0: 1/x, 1: 1/sqrt(x), 2: exp(x), 3: erfc(x), 4: exp(-x^2) as returned together with erfc, 5: log(x), 6: tanh(x) for x >= 0, used by the GENO blend) on n device values. */
 int cgks_debug_math(int which, long n, const double* d_in, double* d_out, void* cuda_stream);
 
 int cgks_destroy(cgks_ctx*);

@@ -636,12 +636,13 @@ __global__ void debug_math_kernel(int which, long n, const double* __restrict__ 
   else if (which == 1) r = drsqrt(x);
   else if (which == 2) r = dexp(x);
   else if (which == 5) r = dlog(x);
+  else if (which == 6) r = dtanh_pos(x);
   else { derfc_exp(x, r, e); if (which == 4) r = e; }
   out[t] = r;
 }
 
 extern "C" int cgks_debug_math(int which, long n, const double* d_in, double* d_out, void* stream) {
-  if (which < 0 || which > 5 || n < 0 || !d_in || !d_out) return CGKS_EINVAL;
+  if (which < 0 || which > 6 || n < 0 || !d_in || !d_out) return CGKS_EINVAL;
   if (n == 0) return CGKS_OK;
   debug_math_kernel<<<(unsigned)((n + 255) / 256), 256, 0, (cudaStream_t)stream>>>(which, n, d_in, d_out);
   return cudaGetLastError() == cudaSuccess ? CGKS_OK : CGKS_ECUDA;

@@ -321,6 +321,8 @@ def test_special_functions_of_the_flux_kernel():
         r = mp.log(mp.mpf(float(a)))
         assert abs(mp.mpf(float(b)) - r) <= 3e-16 * max(abs(r), mp.mpf(1) / 8), a
     np.testing.assert_allclose(gl, np.log(xl), rtol=1e-15, atol=3e-17)
+    xt = np.concatenate([rng.uniform(0.0, 12.0, 20000), 10.0 ** rng.uniform(-8, 0, 5000), [0.0, 5.0, 40.0]])
+    np.testing.assert_allclose(binding.debug_math(6, xt), np.tanh(xt), rtol=0, atol=3e-16)      # the GENO path function: absolute accuracy
     xe = np.concatenate([rng.uniform(-700, 10, 20000), rng.uniform(-1, 1, 20000)])
     np.testing.assert_allclose(binding.debug_math(2, xe), np.exp(xe), rtol=1e-15)
     xu = np.array([-745.0, -760.0, -800.0, -1e5, -1e300])
