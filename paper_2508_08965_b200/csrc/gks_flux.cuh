@@ -295,12 +295,10 @@ __device__ __forceinline__ void gks_flux_local(const GasConst& gc, double dt, do
     lab_acc<false>(g0, MF, G3F);
   }
   // collision time
-  double tau_phys = 0.0;
-  if (gc.mu_ref > 0.0) {
-    double visc = gc.mu_ref;
-    if (gc.omega != 0.0) visc *= dexp(gc.omega * dlog(g0.hil * gc.inv_T_ref));      // (T/T_ref)^omega, T = p/rho
-    tau_phys = visc * (2.0 * g0.lam * g0.irho);                                    // mu / p0
-  }
+  // branch-free: an inviscid run (mu_ref = 0, T_ref possibly unset) evaluates the power law at T/T_ref = 1
+  const double Trel = (gc.mu_ref > 0.0) ? g0.hil * gc.inv_T_ref : 1.0;
+  const double visc = gc.mu_ref * dexp(gc.omega * dlog(Trel));                    // mu_ref (T/T_ref)^omega, T = p/rho
+  const double tau_phys = visc * (2.0 * g0.lam * g0.irho);                        // mu / p0
   const double dpr = ddiv(fabs(pl - pr), fabs(pl + pr));
   const double tau = tau_phys + gc.c1 * dt + gc.c2 * dpr * dt;
   // Time-integrated coefficients of the six groups of Eq. 5 over [0, dt] and [0, dt/2], combined as
@@ -309,9 +307,14 @@ __device__ __forceinline__ void gks_flux_local(const GasConst& gc, double dt, do
   //   c_t = [ w, u - 2 tau w, 1 - tau w, -w, 2 tau w - u, tau w ]           (so the W0 coefficient c_t0 + c_t3 vanishes)
   //   c_n = [ 1 - z, tau (2z - s - 1), -tau (1 - z), z, tau (s - 2z), -tau z ]   (and c_n0 + c_n3 = 1)
   // which avoids the cancellation between the two time integrals.  tau = 0 (reading T2): f = g0 (1 + Abar t).
-  double cn[6] = { 1.0, 0.0, 0.0, 0.0, 0.0, 0.0 }, ct[6] = { 0.0, 0.0, 1.0, 0.0, 0.0, 0.0 };
-  if (tau != 0.0) {
-    const double E = dexp(-0.5 * dt * drcp(tau)), x = 1.0 - E, y = tau * idt;
+  // evaluated without a branch: with tau = 0 the exponential is replaced by its limit E = 0 and y = 0, which gives exactly the
+  // coefficients of the tau = 0 solution, c_n = [1, 0, 0, 0, 0, 0] and c_t = [0, 0, 1, 0, 0, 0]
+  double cn[6], ct[6];
+  {
+    const bool tz = (tau == 0.0);
+    double E = dexp(-0.5 * dt * drcp(tz ? 1.0 : tau));
+    E = tz ? 0.0 : E;
+    const double x = 1.0 - E, y = tau * idt;
     const double w = 4.0 * (y * idt) * (x * x), u = 4.0 * y * (E * x), tw = tau * w;
     ct[0] = w; ct[1] = u - 2.0 * tw; ct[2] = 1.0 - tw; ct[3] = -w; ct[4] = -ct[1]; ct[5] = tw;
     if (!STAGE2) {
@@ -331,7 +334,7 @@ __device__ __forceinline__ void gks_flux_local(const GasConst& gc, double dt, do
     }
   }
   // Prandtl number fix (reading F2): energy flux += (1/Pr - 1) q, q the heat flux of the same distribution
-  if (gc.Pr_fix != 0.0) {
+  {
     const double U0 = g0.U, V0 = g0.V, W0 = g0.W, ke = 0.5 * (U0 * U0 + V0 * V0 + W0 * W0);
     const double qt = Ft[4] - U0 * Qt[4] - U0 * (Ft[1] - U0 * Qt[1]) - V0 * (Ft[2] - U0 * Qt[2]) - W0 * (Ft[3] - U0 * Qt[3]) + ke * (Ft[0] - U0 * Qt[0]);
     Ft[4] += gc.Pr_fix * qt;
