@@ -145,7 +145,7 @@ static cudaError_t set_flux_smem() {
   CGKS_ATTR(false, 0, true); CGKS_ATTR(false, 1, true); CGKS_ATTR(false, 2, true);
   CGKS_ATTR(false, 0, false); CGKS_ATTR(false, 1, false); CGKS_ATTR(false, 2, false);
 #undef CGKS_ATTR
-#define CGKS_ATTR(C, A, ST) if (e == cudaSuccess) e = cudaFuncSetAttribute(sweep_kernel<C, A, ST>, cudaFuncAttributeMaxDynamicSharedMemorySize, sw_smem_bytes(C))
+#define CGKS_ATTR(C, A, ST) if (e == cudaSuccess) e = cudaFuncSetAttribute(sweep_kernel<C, A, ST>, cudaFuncAttributeMaxDynamicSharedMemorySize, sw_smem_bytes(C, A, ST))
   CGKS_ATTR(true, 0, 1); CGKS_ATTR(true, 1, 1); CGKS_ATTR(true, 2, 1);
   CGKS_ATTR(true, 0, 2); CGKS_ATTR(true, 1, 2); CGKS_ATTR(true, 2, 2);
   CGKS_ATTR(false, 0, 1); CGKS_ATTR(false, 1, 1); CGKS_ATTR(false, 2, 1);
@@ -370,8 +370,8 @@ static void launch_sweeps(cgks_ctx* c, const Slab& sl, const double* Win, double
     return (unsigned)(nb < maxb ? nb : maxb);
   };
 #define CGKS_SWEEP(AX) do { const unsigned grid = lines(AX); Timed t(c, KC_FLUX); \
-    if (stage == 2) sweep_kernel<CART, AX, 2><<<grid, SW_TPB, sw_smem_bytes(CART), c->stream>>>(m, sl, sp, Win, c->pv, Wcur, Wstar, Wsave, gc, dt, idt); \
-    else sweep_kernel<CART, AX, 1><<<grid, SW_TPB, sw_smem_bytes(CART), c->stream>>>(m, sl, sp, Win, c->pv, Wcur, Wstar, Wsave, gc, dt, idt); } while (0)
+    if (stage == 2) sweep_kernel<CART, AX, 2><<<grid, SW_TPB, sw_smem_bytes(CART, AX, 2), c->stream>>>(m, sl, sp, Win, c->pv, Wcur, Wstar, Wsave, gc, dt, idt); \
+    else sweep_kernel<CART, AX, 1><<<grid, SW_TPB, sw_smem_bytes(CART, AX, 1), c->stream>>>(m, sl, sp, Win, c->pv, Wcur, Wstar, Wsave, gc, dt, idt); } while (0)
   CGKS_SWEEP(0); CGKS_SWEEP(1); CGKS_SWEEP(2);
 #undef CGKS_SWEEP
 }

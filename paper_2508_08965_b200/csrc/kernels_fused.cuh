@@ -27,12 +27,24 @@ namespace cgks {
 constexpr int SW_TPB = 128;                  // 4 warps; FLUX_MINB blocks per SM (254 registers per thread)
 constexpr int SW_CELLS = 8;                  // cells per warp tile
 constexpr int SW_SMEM_IN = 40 * SW_TPB;      // doubles: staged inputs [20 chunks][SW_TPB][2]
-constexpr int SW_SMEM_RMW = 2 * 10 * SW_TPB; // doubles: read-modify-write operands [2 (step parity)][10][SW_TPB]
-// doubles: hand-over values [20 (+ 4 on general meshes: vector area and area of the face)][SW_TPB]
-__host__ __device__ constexpr int sw_smem_x(bool cart) { return (cart ? 20 : 24) * SW_TPB; }
-// doubles, general meshes only: [2 (step parity)] + face vector area (3), tangent (3), cell volume
+// Shared memory of a block, in doubles (the sizes depend on the kernel: the Cartesian kernels must stay at or below 81 KB per block,
+// the configuration that leaves 92 KB of L1; profiles/r02e_experiments.md):
+//   staged inputs      [20 chunks][SW_TPB][2]
+//   hand-over values   [rows][row length]: rows = 20 (stage 1) or 10 (stage 2: time derivatives only), + 4 on general meshes (vector
+//                      area and area of the face); a row holds one slot per thread, and for AXIS = 0 per warp 8 more in front of its
+//                      32: the values of its last cell of the step before, by step parity (the first cell of a tile takes them)
+//   read-modify-write operands [2 (step parity)][rows][SW_TPB]: rows = 5 for the first direction of stage 1 (Q^n only), else 10
+//   face metrics       general meshes only: [2 (step parity)][7][SW_TPB] (+ face vector area, tangent, cell volume)
+__host__ __device__ constexpr int sw_x_warp(int axis) { return axis == 0 ? 40 : 32; }                 // hand-over slots per warp in a row
+__host__ __device__ constexpr int sw_x_row(int axis) { return sw_x_warp(axis) * (SW_TPB / 32); }
+__host__ __device__ constexpr int sw_x_rows(bool cart, int stage) { return (stage == 2 ? 10 : 20) + (cart ? 0 : 4); }
+__host__ __device__ constexpr int sw_smem_x(bool cart, int axis, int stage) { return sw_x_rows(cart, stage) * sw_x_row(axis); }
+__host__ __device__ constexpr int sw_rmw_rows(int axis, int stage) { return (axis == 0 && stage == 1) ? 5 : 10; }
+__host__ __device__ constexpr int sw_smem_rmw(int axis, int stage) { return 2 * sw_rmw_rows(axis, stage) * SW_TPB; }
 __host__ __device__ constexpr int sw_smem_met(bool cart) { return cart ? 0 : 2 * 7 * SW_TPB; }
-__host__ __device__ constexpr int sw_smem_bytes(bool cart) { return (SW_SMEM_IN + sw_smem_x(cart) + SW_SMEM_RMW + sw_smem_met(cart)) * 8; }
+__host__ __device__ constexpr int sw_smem_bytes(bool cart, int axis, int stage) {
+  return (SW_SMEM_IN + sw_smem_x(cart, axis, stage) + sw_smem_rmw(axis, stage) + sw_smem_met(cart)) * 8;
+}
 
 struct SweepPrm {
   int kA, cnt;       // planes kA .. kA+cnt-1 (wrapped) are updated
@@ -105,8 +117,10 @@ __global__ void __launch_bounds__(SW_TPB, FLUX_MINB) sweep_kernel(Mesh m, Slab s
   extern __shared__ __align__(16) double sm[];
   double* smf = sm;                                      // staged inputs
   double* smx = sm + SW_SMEM_IN;                         // hand-over values
-  double* smr = sm + SW_SMEM_IN + sw_smem_x(CART);       // read-modify-write operands
-  double* smm = sm + SW_SMEM_IN + sw_smem_x(CART) + SW_SMEM_RMW;      // face metrics of the step (general meshes)
+  double* smr = sm + SW_SMEM_IN + sw_smem_x(CART, AXIS, STAGE);       // read-modify-write operands
+  double* smm = smr + sw_smem_rmw(AXIS, STAGE);                       // face metrics of the step (general meshes)
+  constexpr int RR = sw_rmw_rows(AXIS, STAGE);                        // rows of one parity of the read-modify-write operands
+  constexpr int XR = sw_x_row(AXIS);                                  // row length of the hand-over buffer
   const int tid = threadIdx.x, lane = tid & 31, q = lane & 3, cl = lane >> 2;
   const int gw = blockIdx.x * (SW_TPB / 32) + (tid >> 5), nw = gridDim.x * (SW_TPB / 32);
   const long n = m.n;
@@ -131,7 +145,7 @@ __global__ void __launch_bounds__(SW_TPB, FLUX_MINB) sweep_kernel(Mesh m, Slab s
         cp_async8(mt + 6 * SW_TPB, m.met + MET_VOL * n + p.cL);
       }
       if (s >= 0) {
-        double* r = smr + par * (10 * SW_TPB) + tid;
+        double* r = smr + par * (RR * SW_TPB) + tid;
         const long oq = 4 * (long)p.cL + q, sq = 4 * n;
         if (FIRST) {
           if (q == 0) {
@@ -267,45 +281,48 @@ __global__ void __launch_bounds__(SW_TPB, FLUX_MINB) sweep_kernel(Mesh m, Slab s
     double M[4][5];
     double Am[3] = { 0, 0, 0 }, Sm = 0;      // general meshes: vector area and area of the - face (the + face of the cell below)
     {
-      double* xs = smx + tid;
-      auto put = [&]() {
+      // Unconditional: a lane without a cell hands over (and takes) numbers nobody uses.  AXIS = 1, 2: the thread's own slot.
+      // AXIS = 0: the slot of the lane four to the left; the first cell of the tile takes the copy that the last cell of the step
+      // before left in the warp's 2 x 4 front slots (by step parity): no lane-dependent branch around the loads.
+      const int wslot = (tid >> 5) * sw_x_warp(AXIS);
+      double* xs = smx + wslot + (AXIS == 0 ? 8 + lane : lane);
+      auto put = [&](double* dst) {
         if (!CART) {
 #pragma unroll
-          for (int r = 0; r < 3; r++) xs[(20 + r) * SW_TPB] = A[r];
-          xs[23 * SW_TPB] = Sface;
+          for (int r = 0; r < 3; r++) dst[(sw_x_rows(true, STAGE) + r) * XR] = A[r];
+          dst[(sw_x_rows(true, STAGE) + 3) * XR] = Sface;
         }
         if (!STAGE2) {
 #pragma unroll
-          for (int v = 0; v < 5; v++) { xs[v * SW_TPB] = P[0][v]; xs[(5 + v) * SW_TPB] = P[1][v]; xs[(10 + v) * SW_TPB] = R[0][v]; xs[(15 + v) * SW_TPB] = R[1][v]; }
+          for (int v = 0; v < 5; v++) { dst[v * XR] = P[0][v]; dst[(5 + v) * XR] = P[1][v]; dst[(10 + v) * XR] = R[0][v]; dst[(15 + v) * XR] = R[1][v]; }
         } else {
 #pragma unroll
-          for (int v = 0; v < 5; v++) { xs[v * SW_TPB] = P[1][v]; xs[(5 + v) * SW_TPB] = R[1][v]; }
+          for (int v = 0; v < 5; v++) { dst[v * XR] = P[1][v]; dst[(5 + v) * XR] = R[1][v]; }
         }
       };
       auto get = [&](const double* src) {
         if (!CART) {
 #pragma unroll
-          for (int r = 0; r < 3; r++) Am[r] = src[(20 + r) * SW_TPB];
-          Sm = src[23 * SW_TPB];
+          for (int r = 0; r < 3; r++) Am[r] = src[(sw_x_rows(true, STAGE) + r) * XR];
+          Sm = src[(sw_x_rows(true, STAGE) + 3) * XR];
         }
         if (!STAGE2) {
 #pragma unroll
-          for (int v = 0; v < 5; v++) { M[0][v] = src[v * SW_TPB]; M[1][v] = src[(5 + v) * SW_TPB]; M[2][v] = src[(10 + v) * SW_TPB]; M[3][v] = src[(15 + v) * SW_TPB]; }
+          for (int v = 0; v < 5; v++) { M[0][v] = src[v * XR]; M[1][v] = src[(5 + v) * XR]; M[2][v] = src[(10 + v) * XR]; M[3][v] = src[(15 + v) * XR]; }
         } else {
 #pragma unroll
-          for (int v = 0; v < 5; v++) { M[1][v] = src[v * SW_TPB]; M[3][v] = src[(5 + v) * SW_TPB]; }
+          for (int v = 0; v < 5; v++) { M[1][v] = src[v * XR]; M[3][v] = src[(5 + v) * XR]; }
         }
       };
       if (AXIS == 0) {
-        // lane - 4 computed the face below; the first cell of the tile takes the last cell of the previous step
-        if (cl == 0 && act && s >= 0) get(xs + 4 * (SW_CELLS - 1));
+        __syncwarp();      // the neighbours have taken what this lane left in the step before
+        put(xs);
+        if (cl == SW_CELLS - 1) put(smx + wslot + 4 * par + q);
         __syncwarp();
-        if (act) put();
-        __syncwarp();
-        if (cl > 0 && act && s >= 0) get(xs - 4);
+        get(cl == 0 ? smx + wslot + 4 * (par ^ 1) + q : xs - 4);
       } else {
-        if (act && s >= 0) get(xs);
-        if (act) put();
+        get(xs);
+        put(xs);
       }
     }
     if (s >= 0) {
@@ -314,12 +331,13 @@ __global__ void __launch_bounds__(SW_TPB, FLUX_MINB) sweep_kernel(Mesh m, Slab s
       const double* Ap = A; const double Sp = Sface;
       if (CART) cf = 0.25 / m.h[AXIS]; else cf = 0.25 * drcp(smm[par * (7 * SW_TPB) + 6 * SW_TPB + tid]);      // 1/(4 |Omega|)
       const double hdt = 0.5 * dt;
-      const double* rb = smr + par * (10 * SW_TPB) + tid;
+      const double* rb = smr + par * (RR * SW_TPB) + tid;
       const int comp = q - 1;      // gradient component owned by this lane (q = 0: the cell average)
       // this lane's component of the records of variable 0; the next variable is 4 n (records) / 12 n (line differences) further
       const long oq = 4 * (long)cur.cL + q, od = iD(0, AXIS, cur.cL, n) + q;
       double* pq_star = Wstar + oq; double* pq_save = Wsave + oq; double* pd_star = Wstar + od; double* pd_save = Wsave + od;
       const long sq = 4 * n, sd = 12 * n;
+      double o_q0[5], o_q1[5], o_d0[5], o_d1[5];      // what this lane writes: record component and line difference, W* and saved buffer
 #pragma unroll
       for (int v = 0; v < 5; v++) {
         // sums over the four Gauss points of the face pair
@@ -372,31 +390,31 @@ __global__ void __launch_bounds__(SW_TPB, FLUX_MINB) sweep_kernel(Mesh m, Slab s
           sFt = tT; sD[0] = tT; sD[1] = tT; sD[2] = tT;
           if (!STAGE2) { const double tN = rs(kN); sF = tN; sV[0] = tN; sV[1] = tN; sV[2] = tN; }
         }
-        // this lane's component of the record { Q, G_x, G_y, G_z }
+        // this lane's component of the record { Q, G_x, G_y, G_z }: the increments of both kinds are formed and selected (no branch)
         double gV = 0.0, gD = 0.0;      // gradient sums of the values / of the time derivatives, this lane's component
-        if (CART) { if (comp == AXIS) { gV = sV[0]; gD = sD[0]; } }
-        else {
-          if (comp == 0) { gV = sV[0]; gD = sD[0]; } else if (comp == 1) { gV = sV[1]; gD = sD[1]; } else if (comp == 2) { gV = sV[2]; gD = sD[2]; }
-        }
+        if (CART) { gV = (comp == AXIS) ? sV[0] : 0.0; gD = (comp == AXIS) ? sD[0] : 0.0; }
+        else { gV = sV[0]; gD = sD[0]; }      // the reduce-scatter left this lane's kind in every entry
         if (!STAGE2) {
-          double inc_star, inc_save;
-          if (q == 0) { inc_star = -cf * (hdt * sF + 0.125 * dt * dt * sFt); inc_save = -cf * (dt * sF + (1.0 / 6.0) * dt * dt * sFt); }
-          else { inc_star = cf * (gV + hdt * gD); inc_save = cf * gV; }
-          double b_star, b_save;
-          if (FIRST) { b_star = (q == 0) ? rb[v * SW_TPB] : 0.0; b_save = b_star; }
-          else { b_star = rb[v * SW_TPB]; b_save = rb[(5 + v) * SW_TPB]; }
-          if (act) {
-            pq_star[v * sq] = b_star + inc_star;
-            pq_save[v * sq] = b_save + inc_save;
-            pd_star[v * sd] = d0 + hdt * d1;
-            pd_save[v * sd] = d0;
-          }
+          const double iq_star = -cf * (hdt * sF + 0.125 * dt * dt * sFt), iq_save = -cf * (dt * sF + (1.0 / 6.0) * dt * dt * sFt);
+          const double ig_star = cf * (gV + hdt * gD), ig_save = cf * gV;
+          const double b0 = rb[v * SW_TPB];
+          const double b_star = FIRST ? (q == 0 ? b0 : 0.0) : b0;
+          const double b_save = FIRST ? b_star : rb[(RR - 5 + v) * SW_TPB];
+          o_q0[v] = b_star + (q == 0 ? iq_star : ig_star);
+          o_q1[v] = b_save + (q == 0 ? iq_save : ig_save);
+          o_d0[v] = d0 + hdt * d1;
+          o_d1[v] = d0;
         } else {
           const double inc = (q == 0) ? -cf * ((1.0 / 3.0) * dt * dt * sFt) : cf * (dt * gD);
-          if (act) {
-            pq_save[v * sq] = rb[v * SW_TPB] + inc;
-            pd_save[v * sd] = rb[(5 + v) * SW_TPB] + dt * d1;
-          }
+          o_q1[v] = rb[v * SW_TPB] + inc;
+          o_d1[v] = rb[(5 + v) * SW_TPB] + dt * d1;
+        }
+      }
+      if (act) {
+#pragma unroll
+        for (int v = 0; v < 5; v++) {
+          if (!STAGE2) { pq_star[v * sq] = o_q0[v]; pd_star[v * sd] = o_d0[v]; }
+          pq_save[v * sq] = o_q1[v]; pd_save[v * sd] = o_d1[v];
         }
       }
     }
