@@ -28,26 +28,26 @@ UNIT = "cell-updates/s"
 # Dominant kernel = sweep_kernel (gas-kinetic flux + update/S2O4 combine of one face direction, csrc/kernels_fused.cuh), bound by
 # the plain FP64 ALUs.  Two flop counts per face Gauss point (FMA = 2, add/mul = 1), DESIGN.md section 7.2:
 #  * EXECUTED by the formulation as built (primed-basis moments, own reciprocal / rsqrt / exp / erfc of csrc/fastmath64.cuh, the
-#    quad sums and the combine), from ncu's executed-FP64-op counters on the committed capture profiles/r02g_kernels_128.md,
+#    quad sums and the combine), from ncu's executed-FP64-op counters on the committed capture profiles/r02k_final.md,
 #    per point of an updated cell (the extra first face of every line of a sweep is NOT counted as useful work): stage 1
 #    computes F, F_t, Q, Q_t and both one-sided values, stage 2 only the time derivatives.  This is the leanest formulation
 #    known to the authors of this repository and is what `roofline.achieved` uses: it can only understate the algorithmic work.
 #  * ORACLE-COUNTED (counting-double build of the CPU oracle, oracle/flop_count.py; operations on non-zero
 #    operands): the oracle evaluates every term of Eq. 5 with the generic moment routine and needs 7x the arithmetic, so
 #    a fraction formed with it exceeds 1; it is printed beside the other, not used as the numerator.
-SWEEP_FLOPS_STAGE1 = 2263.0         # per point: 833 DFMA + 459 DMUL + 137 DADD = 1429 FP64 instructions (flux solver ~2175, quad sums and combine ~90)
-SWEEP_FLOPS_STAGE2 = 2071.0         # per point: 762 DFMA + 442 DMUL + 103 DADD = 1308 FP64 instructions (flux solver ~2025, quad sums and combine ~45)
+SWEEP_FLOPS_STAGE1 = 2286.0         # per point: 843 DFMA + 471 DMUL + 128 DADD = 1442 FP64 instructions (flux solver ~2180, quad sums and combine ~105)
+SWEEP_FLOPS_STAGE2 = 2069.0         # per point: 765 DFMA + 440 DMUL + 99 DADD = 1304 FP64 instructions (flux solver ~2025, quad sums and combine ~45)
 FLUX_SOURCE_SHA16 = "457dec422c688e16"      # sha256 (16 hex digits) of gks_flux.cuh + fastmath64.cuh + math_gen.cuh + kernels_fused.cuh the counts were taken on
 FLUX_FLOPS_ORACLE = 15584.0          # tests/test_abi.py checks this constant against oracle/flop_count.py
 # Round 1's flux kernel executed 3092.7 / 2923.2 flops per point for the same result (profiles/r01d_kernels_128.md); VERDICT r1's
 # target "frac >= 0.50, i.e. flux <= 223 ms per step" is stated in that count, so the fraction in that count is printed too.
 FLUX_FLOPS_R01 = (3092.7, 2923.2)
-SWEEP_FP64_PIPE_ACTIVE_NCU = (0.572, 0.602)     # sm__pipe_fp64_cycles_active of the stage-1 / stage-2 launches, same capture
+SWEEP_FP64_PIPE_ACTIVE_NCU = (0.621, 0.656)     # sm__pipe_fp64_cycles_active of the stage-1 / stage-2 launches, same capture
 # Bytes per point.  Algorithmic: 2 x 20 reconstructed inputs (320 B) + the state records the direction reads and writes, per
 # cell and stage 1: 40 (Q^n) + 2 x 320 read, 3 x 640 written; stage 2: 3 x 320 read, 3 x 320 written; / 12 points.
 # Measured: dram__bytes_read + write per launch / points, same capture.
 SWEEP_BYTES_ALG = (320.0 + (40 + 640 + 1920) / 12.0, 320.0 + (960 + 960) / 12.0)
-SWEEP_TRAFFIC = (556.3, 490.9)
+SWEEP_TRAFFIC = (556.1, 490.7)
 FP64_PEAK_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12      # SMs x FP64 FMA lanes x 2 x max SM clock = 37.2
 
 
@@ -318,7 +318,7 @@ def run_ours(args):
                               "term-by-term evaluation needs 7x the arithmetic, so its count would give a fraction above 1 (DESIGN.md 7.2)",
                 "traffic": 0.5 * sum(SWEEP_TRAFFIC) * pts_per_launch,
                 "algorithmic_bytes": alg_bytes_launch,
-                "traffic_note": "bytes per average launch = ncu dram bytes per point (profiles/r02g_kernels_128.md) x points per launch; "
+                "traffic_note": "bytes per average launch = ncu dram bytes per point (profiles/r02k_final.md) x points per launch; "
                                 "algorithmic bytes per point %.0f (stage 1) / %.0f (stage 2)" % SWEEP_BYTES_ALG,
                 "peak_source": "HBM: " + hbm_peak[1] + "; FP64: derived, 148 SMs x 64 FP64 FMA lanes x 2 x 1.965 GHz (DESIGN.md section 7), "
                                "MEASURED_PEAKS.json has no FP64 entry",

@@ -116,7 +116,7 @@ def test_flux_flop_constant_is_the_oracle_count():
 
 def test_flux_flop_constants_belong_to_the_committed_kernel_source():
     """bench.py's executed-flop constants were counted with ncu on a specific revision of the flux arithmetic
-    and of the sweep kernel around it (profiles/r02g_kernels_128.md); a change to gks_flux.cuh / fastmath64.cuh / math_gen.cuh /
+    and of the sweep kernel around it (profiles/r02k_final.md); a change to gks_flux.cuh / fastmath64.cuh / math_gen.cuh /
     kernels_fused.cuh without a re-count fails here."""
     import hashlib
     import importlib.util
