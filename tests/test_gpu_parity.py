@@ -152,7 +152,8 @@ def test_slab_pipeline_equals_resident():
     full, _ = parity.run_gpu(w, 2)
     n = 12 ** 3
     fixed = 3 * 80 * n * 8 + 5 * n * 8 + 37 * n * 8 + 4096
-    budget = fixed + 6 * 480 * 144 * 8                   # 6 slots of reconstructed face values -> slab depth 4 -> 3 chunks
+    slot = 480 + (360 if os.environ.get("CGKS_PIPELINE") == "split" else 0)      # the three-kernel pipeline also holds face fluxes
+    budget = fixed + 6 * slot * 144 * 8                  # 6 slots of reconstructed face values -> slab depth 4 -> 3 chunks
     s = binding.Solver(w["nodes"], binding.make_params(**w["params"], nonlinear=1), budget_bytes=budget)
     assert s.slab_depth() == 4
     s.close()
@@ -200,7 +201,8 @@ def test_sweep_lines_cut_into_segments():
     _check(w, 1, TOL_1)
     full, _ = parity.run_gpu(w, 2)
     n = shape[0] * shape[1] * shape[2]; plane = shape[0] * shape[1]
-    budget = 3 * 80 * n * 8 + 5 * n * 8 + 37 * n * 8 + 4096 + 30 * 480 * plane * 8
+    slot = 480 + (360 if os.environ.get("CGKS_PIPELINE") == "split" else 0)
+    budget = 3 * 80 * n * 8 + 5 * n * 8 + 37 * n * 8 + 4096 + 30 * slot * plane * 8
     s = binding.Solver(w["nodes"], binding.make_params(**w["params"], nonlinear=1), budget_bytes=budget)
     assert 24 < s.slab_depth() < shape[2]          # two chunks, the first longer than the shortest segment
     s.close()
