@@ -387,7 +387,8 @@ static void run_stage(cgks_ctx* c, int stage, double dt) {
     const long nt = (long)cnt * m.plane;
     dim3 grid((unsigned)((nt + TPB - 1) / TPB), 5);
     Timed t(c, KC_RECON);
-    recon_kernel<CART><<<grid, TPB, 0, c->stream>>>(m, sl, Win, c->pv, c->chi, rp, kA, nt, c->d_flags + 3);
+    if (rp.nonlinear) recon_kernel<CART, false, true><<<grid, TPB, 0, c->stream>>>(m, sl, Win, c->pv, c->chi, rp, kA, nt, c->d_flags + 3);
+    else recon_kernel<CART, false, false><<<grid, TPB, 0, c->stream>>>(m, sl, Win, c->pv, c->chi, rp, kA, nt, c->d_flags + 3);
   };
   auto update = [&](int kA, int cnt) {
     const long nt = (long)cnt * m.plane;
@@ -491,8 +492,8 @@ extern "C" int cgks_debug_stage(cgks_ctx* c, double dt, double* d_pv, double* d_
   const long nt = m.n;
   dim3 grid((unsigned)((nt + TPB - 1) / TPB), 5);
   const double* Win = c->W[c->cur];
-  if (m.cart) recon_kernel<true><<<grid, TPB, 0, c->stream>>>(m, sl, Win, c->pv, c->chi, rp, 0, nt, c->d_flags + 3);
-  else recon_kernel<false><<<grid, TPB, 0, c->stream>>>(m, sl, Win, c->pv, c->chi, rp, 0, nt, c->d_flags + 3);
+  if (m.cart) { if (rp.nonlinear) recon_kernel<true, false, true><<<grid, TPB, 0, c->stream>>>(m, sl, Win, c->pv, c->chi, rp, 0, nt, c->d_flags + 3); else recon_kernel<true, false, false><<<grid, TPB, 0, c->stream>>>(m, sl, Win, c->pv, c->chi, rp, 0, nt, c->d_flags + 3); }
+  else { if (rp.nonlinear) recon_kernel<false, false, true><<<grid, TPB, 0, c->stream>>>(m, sl, Win, c->pv, c->chi, rp, 0, nt, c->d_flags + 3); else recon_kernel<false, false, false><<<grid, TPB, 0, c->stream>>>(m, sl, Win, c->pv, c->chi, rp, 0, nt, c->d_flags + 3); }
   c->launches++;
   if (d_pv) { pv_unpack_kernel<<<dim3((unsigned)((nt + TPB - 1) / TPB), 24 * NVAR), TPB, 0, c->stream>>>(sl, m.n, c->pv, d_pv); c->launches++; }
   if (d_fx && !c->fx) return fail(c, CGKS_ENOMEM, "flux tap: the workspace has no room for the face-flux buffer");
@@ -520,7 +521,8 @@ static void run_diagnostics(cgks_ctx* c, double* d_acc) {
     sl.kbase = k0;
     const long nt = (long)cnt * m.plane;
     const unsigned nb = (unsigned)((nt + TPB - 1) / TPB);
-    { Timed t(c, KC_OTHER); recon_kernel<CART, true><<<dim3(nb, 5), TPB, 0, c->stream>>>(m, sl, Win, c->pv, nullptr, rp, k0, nt, c->d_flags + 3); }
+    { Timed t(c, KC_OTHER); if (rp.nonlinear) recon_kernel<CART, true, true><<<dim3(nb, 5), TPB, 0, c->stream>>>(m, sl, Win, c->pv, nullptr, rp, k0, nt, c->d_flags + 3);
+      else recon_kernel<CART, true, false><<<dim3(nb, 5), TPB, 0, c->stream>>>(m, sl, Win, c->pv, nullptr, rp, k0, nt, c->d_flags + 3); }
     { Timed t(c, KC_OTHER); diag_kernel<CART><<<nb, TPB, 0, c->stream>>>(m, sl, Win, c->pv, dp, k0, nt, scratch); }
     { Timed t(c, KC_OTHER); diag_reduce_kernel<<<1, 256, 0, c->stream>>>(scratch, (long)nb, d_acc); }
   }

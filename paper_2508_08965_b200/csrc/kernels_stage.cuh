@@ -93,7 +93,9 @@ __device__ __forceinline__ void recon_gather_axis(const ReconCell<CART>& rc, con
 
 // VOLUME = true: the same polynomial evaluated at the 8 interior points (+-g, +-g, +-g) of the 2x2x2 Gauss rule instead
 // (pv planes 0..7, used by the diagnostics of PAPER.md:428-454).
-template <bool CART, bool VOLUME = false>
+// NL: the GENO blend is compiled in (nonlinear = 1, the paper's default) or out (linear scheme), so that the thread is one block of
+// straight-line code either way.
+template <bool CART, bool VOLUME = false, bool NL = true>
 __global__ void __launch_bounds__(128, 3) recon_kernel(Mesh m, Slab sl, const double* __restrict__ W, double* __restrict__ pv,
                                                     double* __restrict__ chi_out, ReconPrm rp, int kA, long nthreads,
                                                     int* __restrict__ flag) {
@@ -131,7 +133,7 @@ __global__ void __launch_bounds__(128, 3) recon_kernel(Mesh m, Slab sl, const do
     la[2] = 0.25 * (Dl[0] + Dl[1] + Dl[2] + Dl[3]); acc_line<2>(Dl, a);
   }
   double chi = 1.0;
-  if (rp.nonlinear) {
+  if (NL) {
     // six linear polynomials (Eq. 15): normal slope = average difference, tangential = mean line difference
     double wsum = 0.0, bw[3] = { 0, 0, 0 };
 #pragma unroll
