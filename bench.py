@@ -37,7 +37,7 @@ UNIT = "cell-updates/s"
 #    a fraction formed with it exceeds 1; it is printed beside the other, not used as the numerator.
 SWEEP_FLOPS_STAGE1 = 2286.0         # per point: 843 DFMA + 471 DMUL + 128 DADD = 1442 FP64 instructions (flux solver ~2180, quad sums and combine ~105)
 SWEEP_FLOPS_STAGE2 = 2069.0         # per point: 765 DFMA + 440 DMUL + 99 DADD = 1304 FP64 instructions (flux solver ~2025, quad sums and combine ~45)
-FLUX_SOURCE_SHA16 = "457dec422c688e16"      # sha256 (16 hex digits) of gks_flux.cuh + fastmath64.cuh + math_gen.cuh + kernels_fused.cuh the counts were taken on
+FLUX_SOURCE_SHA16 = "944b1a218fc1b5cf"      # sha256 (16 hex digits) of gks_flux.cuh + fastmath64.cuh + math_gen.cuh + kernels_fused.cuh the counts were taken on
 FLUX_FLOPS_ORACLE = 15584.0          # tests/test_abi.py checks this constant against oracle/flop_count.py
 # Round 1's flux kernel executed 3092.7 / 2923.2 flops per point for the same result (profiles/r01d_kernels_128.md); VERDICT r1's
 # target "frac >= 0.50, i.e. flux <= 223 ms per step" is stated in that count, so the fraction in that count is printed too.

@@ -9,10 +9,11 @@
 // Mapping.  A WARP owns a tile of 8 cells along i x the 4 Gauss points of their + face of direction AXIS (lane = 4 cell + q)
 // and marches along a line of such tiles in the direction AXIS, one tile per step.  The face computed in the previous step
 // is the - face of the cells of this step: what it hands over (F^n, F_t^n and the right-hand interface values, 20 numbers
-// per point) stays in shared memory -- for AXIS = 1, 2 in the thread's own slot, for AXIS = 0 in the slot of the lane four to
-// the right (the first cell of a tile takes the last cell of the previous tile).  Every line starts with one extra step (the
-// face below its first cell: for AXIS = 0 the periodic image of the row's last face, computed by four lanes).
-// The sums over the four Gauss points of a face (Eq. 8-9) are two butterfly shuffles inside the quad; lane q then owns
+// per point) stays in shared memory -- for AXIS = 1, 2 in the thread's own slot; for AXIS = 0 a lane takes the slot of the lane
+// four to its left, and the first cell of a tile takes a copy that the last cell of the step before left in front slots of the
+// warp's row (by step parity), so the exchange has no lane-dependent branch.  Every line starts with one extra step (the face
+// below its first cell: for AXIS = 0 the periodic image of the row's last face, computed by four lanes).
+// The sums over the four Gauss points of a face (Eq. 8-9) are a reduce-scatter inside the quad (two shuffle rounds); lane q then owns
 // component q of the cell's record { Q, G_x, G_y, G_z } and line difference 4 AXIS + q of the 12 (Eq. 10): a quad reads and
 // writes whole 32-byte sectors.  Direction 0 of stage 1 writes the records, the later directions (and every direction of stage
 // 2, which updates the saved buffer in place) read-modify-write them; these operands are prefetched with cp.async together
