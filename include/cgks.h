@@ -77,6 +77,33 @@ int cgks_get_state(cgks_ctx*, double* d_Q, double* d_G, double* d_D);
    DESIGN.md reading S3).  Synchronises; returns CGKS_ENONPHYSICAL if an earlier stage flagged a bad cell. */
 int cgks_compute_dt(cgks_ctx*, double cfl, double* dt_host);
 
+/* The same time step (reading S3) WITHOUT a context, a workspace or any device allocation, for
+   callers that cannot get device memory: code that is handed a Q array inside a process whose framework allocator already
+   holds all of HBM (a raw cudaMalloc fails there, and so would the workspace cgks_create needs), and time loops that must
+   never stall (cudaMalloc / cudaFree synchronise the device).  The reduction's scratch memory is an array built into the
+   library image: 33 024 bytes on every GPU that loads libcgks.so, held until the process exits.
+     d_Q      DEVICE [5][nk][nj][ni] cell averages (rho, rho U, rho V, rho W, rho E), read only
+     h_host   HOST   [3] cell sizes of a UNIFORM CARTESIAN mesh (period / n per direction, as cgks_create derives them);
+                     general meshes need the metrics of a context: use cgks_compute_dt
+     params   HOST   gamma, mu_ref, visc_omega, T_ref are used
+     d_dt     DEVICE [1] result; +inf when no cell is admissible
+     d_bad    DEVICE [1] or NULL: 1 if a cell average with rho <= 0 or p <= 0 was met (such cells are skipped), else 0
+   Limit: ni * nj * nk <= CGKS_STATIC_MAX_CELLS (256^3); more returns CGKS_EINVAL with a message that says so.  The call
+   enqueues one memset and two kernels on `cuda_stream` and returns without waiting; it calls no cudaMalloc, cudaFree or
+   other allocating routine.  The result does not depend on the device's SM count (one partial minimum per 4096 cells) and
+   is bit-identical to cgks_compute_dt on the same mesh and state as long as both compile to the same per-cell arithmetic
+   (tested to 1e-13).
+   Set-up: the first call on each device (with that device current) looks up the array's device address with
+   cudaGetSymbolAddress, which may load the CUDA module; make that first call before any stream capture begins.
+   Sharing: all calls on one device use the same array.  A call clears the one word that must start at zero and overwrites
+   every partial it reads, so calls that follow each other on one stream are independent; calls that may OVERLAP on the
+   GPU (different streams, or several host threads) race on it and give undefined results -- serialise them.
+   Errors: CGKS_EINVAL / CGKS_ECUDA, message from cgks_static_last_error() (per host thread). */
+enum { CGKS_STATIC_MAX_CELLS = 1 << 24 };
+int cgks_compute_dt_static(int ni, int nj, int nk, const double* d_Q, const double* h_host, const cgks_params* params,
+                           double cfl, double* d_dt, int* d_bad, void* cuda_stream);
+const char* cgks_static_last_error(void);
+
 /* One two-stage fourth-order step of size dt.  Asynchronous.
    Per stage: one reconstruction kernel (Eq. 11-19), then one sweep kernel per face direction that computes the gas-kinetic
    flux at the face Gauss points (Eq. 1-7) and accumulates Eq. 8-10 and the S2O4 combine into the state buffers.  With

@@ -46,6 +46,9 @@ def lib():
         L.cgks_set_state.argtypes = [_vp, _vp, _vp, _vp]
         L.cgks_get_state.argtypes = [_vp, _vp, _vp, _vp]
         L.cgks_compute_dt.argtypes = [_vp, C.c_double, C.POINTER(C.c_double)]
+        L.cgks_compute_dt_static.argtypes = [C.c_int, C.c_int, C.c_int, _vp, C.POINTER(C.c_double), C.POINTER(cgks_params),
+                                             C.c_double, _vp, _vp, _vp]
+        L.cgks_static_last_error.restype = C.c_char_p
         L.cgks_step.argtypes = [_vp, C.c_double]
         L.cgks_stage.argtypes = [_vp, C.c_int, C.c_double]
         L.cgks_create_slab.argtypes = [C.POINTER(_vp), C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, _vp, C.POINTER(cgks_params), _vp, C.c_size_t, _vp]
@@ -83,6 +86,34 @@ def workspace_bytes(ni, nj, nk, budget_bytes=0):
     if rc:
         raise CgksError(rc, "cgks_workspace_bytes")
     return out.value
+
+
+STATIC_MAX_CELLS = 1 << 24
+
+
+def compute_dt_static(Q, h, params, cfl, out_dt, out_bad=None):
+    """cgks_compute_dt_static: the CFL time step of the cell averages Q (5, nk, nj, ni) on a uniform Cartesian mesh of
+    cell sizes h = (hx, hy, hz), without a Solver, a workspace or any device allocation -- for callers that cannot
+    allocate (all of HBM owned by someone else's allocator, or a loop that must not hit cudaMalloc's device-wide
+    synchronisation).  Nothing is allocated here either: Q must already be a contiguous float64 CUDA tensor, and the
+    results go into tensors the caller owns, out_dt (1 float64) and, if given, out_bad (1 int32: 1 when a cell with
+    rho <= 0 or p <= 0 was met).  Asynchronous on the current stream of Q's device.  At most STATIC_MAX_CELLS cells;
+    calls that may overlap on the GPU race on the library's built-in scratch array (include/cgks.h)."""
+    if not (Q.is_cuda and Q.dtype == torch.float64 and Q.is_contiguous() and Q.dim() == 4 and Q.shape[0] == 5):
+        raise ValueError("Q must be a contiguous float64 CUDA tensor of shape (5, nk, nj, ni)")
+    if not (out_dt.is_cuda and out_dt.dtype == torch.float64 and out_dt.numel() >= 1):
+        raise ValueError("out_dt must be a float64 CUDA tensor")
+    if out_bad is not None and not (out_bad.is_cuda and out_bad.dtype == torch.int32 and out_bad.numel() >= 1):
+        raise ValueError("out_bad must be an int32 CUDA tensor")
+    nk, nj, ni = (int(s) for s in Q.shape[1:])
+    prm = params if isinstance(params, cgks_params) else make_params(**params)
+    hh = (C.c_double * 3)(*[float(x) for x in h])
+    with torch.cuda.device(Q.device):
+        st = torch.cuda.current_stream()
+        rc = lib().cgks_compute_dt_static(ni, nj, nk, _ptr(Q), hh, C.byref(prm), float(cfl), _ptr(out_dt), _ptr(out_bad),
+                                          _vp(st.cuda_stream))
+    if rc:
+        raise CgksError(rc, lib().cgks_static_last_error().decode())
 
 
 def fp64_peak_tflops(device="cuda:0"):

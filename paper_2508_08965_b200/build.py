@@ -6,7 +6,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libcgks.so")
-SOURCES = ["cgks_api.cu"]
+SOURCES = ["cgks_api.cu", "cgks_static.cu"]
 HEADERS = ["cgks_common.cuh", "kernels_setup.cuh", "kernels_stage.cuh", "kernels_fused.cuh", "gks_flux.cuh", "fastmath64.cuh", "recon_gen.cuh", "math_gen.cuh"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared"]
