@@ -124,7 +124,10 @@ int cgks_stage(cgks_ctx*, int stage, double dt);
    context holds it.  Before EACH stage the halo planes of the stage's input state must be current:
        cgks_pack_halo(side) on the neighbour  ->  transport (NCCL / peer copy; the caller's)  ->  cgks_unpack_halo(side),
    side 0 = low k, 1 = high k; pack copies the two outermost OWNED planes of that side, unpack fills the two HALO planes
-   of that side, all 80 fields, buffer layout [80][2][nj][ni] (cgks_halo_bytes).  Between cgks_stage(1) and cgks_stage(2)
+   of that side, all 80 fields.  The buffer (cgks_halo_bytes = 80 * 2 * nj * ni doubles) is OPAQUE: it is meant to be moved, not
+   read.  (Its actual order is the library's internal record layout, 20 runs of [2][nj][ni][4]: runs 0..4 hold { Q_v, G_v } of
+   variable v, runs 5..19 the four line differences of (variable, axis) = ((a-5)/3, (a-5)%3); it is NOT [80][2][nj][ni] in the user
+   field order and may change between versions -- fill it only with cgks_pack_halo.)  Between cgks_stage(1) and cgks_stage(2)
    the calls act on the stage state, otherwise on the current state.  cgks_set_state / cgks_get_state take arrays of
    nk_owned + 4 planes (halo planes of Q should hold the neighbours' values so that the bootstrap of reading S2 is right
    on the owned planes; halo planes returned by cgks_get_state are not current).  cgks_compute_dt reduces over the owned

@@ -227,7 +227,8 @@ class Solver:
         self._check(lib().cgks_stage(self._h, int(stage), float(dt)))
 
     def halo_buffer(self):
-        """A device buffer for one side's halo planes, [80][2][nj][ni] (cgks_halo_bytes)."""
+        """A device buffer for one side's halo planes: 80 * 2 * nj * ni doubles (cgks_halo_bytes), opaque -- the library's internal
+        record order, to be filled by pack_halo and read by unpack_halo only (include/cgks.h)."""
         nb = C.c_size_t(0)
         self._check(lib().cgks_halo_bytes(self._h, C.byref(nb)))
         return torch.empty(nb.value // 8, dtype=torch.float64, device=self.device)

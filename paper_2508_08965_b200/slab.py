@@ -13,7 +13,11 @@ import torch.distributed as dist
 
 from . import binding
 
-UP, DOWN = 0, 1          # message tags: sender's HIGH planes -> receiver's LOW halo; sender's LOW planes -> receiver's HIGH halo
+# Message tags, for backends that honour them (gloo, MPI): sender's HIGH planes -> receiver's LOW halo and the reverse.  NCCL's
+# point-to-point calls IGNORE tags: messages between one pair of ranks are matched purely by the order in which they are
+# posted.  exchange_halos therefore never has two messages in flight in the same direction between the same pair (see there);
+# the tags are decoration, not what keeps the ring unambiguous.
+UP, DOWN, BOTH = 0, 1, 2
 
 
 def partition(nk, world):
@@ -48,8 +52,20 @@ def exchange_halos(sub, rank, world, group=None):
     if world == 1:
         sub.unpack_halo(0, send_hi); sub.unpack_halo(1, send_lo)
         return
-    recv_lo, recv_hi = sub.halo_buffer(), sub.halo_buffer()
     lo, hi = neighbours(rank, world)
+    if lo == hi:
+        # world == 2: both neighbours are the SAME rank.  Two sends to one peer would be told apart only by tag (ignored by NCCL)
+        # or by posting order (an invariant nobody can see at the call site), so both halves travel in ONE message per
+        # direction: [low owned planes | high owned planes].  The peer's high planes fill my low halo and the reverse.
+        n = send_lo.numel()
+        send = torch.cat([send_lo, send_hi]); recv = torch.empty_like(send)
+        ops = [dist.P2POp(dist.isend, send, hi, group, BOTH), dist.P2POp(dist.irecv, recv, hi, group, BOTH)]
+        for req in dist.batch_isend_irecv(ops):
+            req.wait()
+        sub.unpack_halo(0, recv[n:]); sub.unpack_halo(1, recv[:n])
+        return
+    # world >= 3: lo != hi, one message per (peer, direction); nothing to disambiguate, whatever the backend does with tags
+    recv_lo, recv_hi = sub.halo_buffer(), sub.halo_buffer()
     ops = [dist.P2POp(dist.isend, send_hi, hi, group, UP), dist.P2POp(dist.isend, send_lo, lo, group, DOWN),
            dist.P2POp(dist.irecv, recv_lo, lo, group, UP), dist.P2POp(dist.irecv, recv_hi, hi, group, DOWN)]
     for req in dist.batch_isend_irecv(ops):

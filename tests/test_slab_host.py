@@ -1,8 +1,9 @@
 """Host-side logic of the slab decomposition (paper_2508_08965_b200/slab.py): partition,
 ring neighbours, periodic halo slices, and the message choreography of exchange_halos / global_min under torch.distributed
-with the gloo backend, world sizes 2 and 3, on CPU.  The sub-domain here is a test double with the library's halo layout
-([80][2][plane]; pack = two outermost owned planes, unpack = two halo planes); the kernels themselves are covered by
-tests/test_gpu_slab.py."""
+with the gloo backend, world sizes 2 and 3, on CPU.  The sub-domain here is a test double with the library's halo SEMANTICS
+(pack = two outermost owned planes, unpack = two halo planes, a buffer of 80 * 2 * plane doubles); the order inside the buffer
+is the double's own ([80][2][plane]) -- the library's is opaque and different (include/cgks.h), and slab.py never looks inside.
+The kernels themselves are covered by tests/test_gpu_slab.py."""
 import os
 import socket
 
@@ -83,12 +84,26 @@ def _worker(rank, world, port, nk, plane, out):
     try:
         k0, cnt = slab.partition(nk, world)[rank]
         s = MockSub(k0, cnt, nk, plane)
+        # NCCL matches point-to-point messages between a pair of ranks by posting order and ignores tags (gloo honours them, so
+        # this test cannot see a tag dependence directly): check instead that no exchange ever posts two messages in the same
+        # direction to the same peer, and that every tag is overwritten with one value before posting
+        posted = []
+        real_batch = dist.batch_isend_irecv
+
+        def spy(ops):
+            posted.append(sorted((op.op.__name__, op.peer) for op in ops))
+            for op in ops:
+                op.tag = 7
+            return real_batch(ops)
+        dist.batch_isend_irecv = spy
         for _ in range(2):                               # twice: the exchange must be repeatable (stage 1, stage 2)
             s.W[:, :2] = -1.0; s.W[:, -2:] = -1.0
             slab.exchange_halos(s, rank, world)
             ok = torch.equal(s.W, s.exact)
+        dist.batch_isend_irecv = real_batch
+        unambiguous = all(len(set(p)) == len(p) for p in posted) and len(posted) == 2
         dt = slab.global_min(0.5 + 0.25 * ((rank + 1) % world), torch.device("cpu"))
-        out[rank] = (bool(ok), dt)
+        out[rank] = (bool(ok) and unambiguous, dt)
     finally:
         dist.destroy_process_group()
 
