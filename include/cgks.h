@@ -149,7 +149,12 @@ int cgks_unpack_halo(cgks_ctx*, int side, const double* d_buf);
      CGKS_BC_OUTFLOW     zero-gradient extrapolation of the outermost owned plane
      CGKS_BC_FARFIELD    the uniform state far_state_host[5] (host pointer: rho, rho U, rho V, rho W, rho E)
    Uniform Cartesian meshes only (CGKS_EINVAL otherwise).  A domain bounded in k on both sides is the sub-domain
-   cgks_create_slab(..., k0 = 0, nk_owned = nk_global, ...) with this call on both sides. */
+   cgks_create_slab(..., k0 = 0, nk_owned = nk_global, ...) with this call on both sides.
+   Initial state of a bounded domain: the bootstrap of cgks_set_state (G = D = NULL, reading S2) runs BEFORE any boundary rule
+   and differences the Q the caller put in the halo planes.  The caller must therefore fill the halo planes of Q consistently
+   with the boundary (mirror image for walls, copies for outflow, the far state), not with the periodic wrap: with periodic
+   images across a wall, the derivative dof of the two owned planes next to it start from the wrong neighbour values unless the
+   data happen to be mirror-symmetric.  Passing G and D explicitly avoids the question. */
 enum { CGKS_BC_SLIP_WALL = 0, CGKS_BC_NOSLIP_WALL = 1, CGKS_BC_OUTFLOW = 2, CGKS_BC_FARFIELD = 3 };
 int cgks_fill_halo_bc(cgks_ctx*, int side, int kind, const double* far_state_host);
 

@@ -39,7 +39,7 @@ static int    g_ready = 0;
    directions, G2 variant B); nothing but that script and its test changes them. */
 static int    g_r5_normalised = 1;   /* R5: 1 tau2 = o/sqrt 2 (unit vector), 0 tau2 = o                               */
 static int    g_s3_sum = 1;          /* S3: 1 rate = sum over directions, 0 rate = max over directions               */
-static int    g_g2_variant = 1;      /* G2: 1 (B) IS^tau = third+fourth derivative part, 0 (A) IS^tau = |IS^H - IS^L| */
+static int    g_g2_variant = 1;      /* G2: 1 (B) IS^tau = third+fourth derivative part, 0 (A) IS^tau = |IS^H - IS^L|, 2 fourth part only */
 void cgks_ref_set_readings(int r5_normalised, int s3_sum, int g2_variant) {
   if (r5_normalised != g_r5_normalised) g_ready = 0;      /* M is rebuilt at the next use */
   g_r5_normalised = r5_normalised; g_s3_sum = s3_sum; g_g2_variant = g2_variant;
@@ -245,7 +245,8 @@ void cgks_ref_recon_reference(const cgks_ref_params* p, const double* d, double*
     /* path function (readings G2: IS^tau = third+fourth derivative part, G3: C = geno_C) */
     double IS4[4]; cgks_ref_smoothness(a, IS4);
     double ISH = IS4[0] + IS4[1] + IS4[2] + IS4[3], ISL = IS4[0], ISt = IS4[2] + IS4[3];
-    if (!g_g2_variant) ISt = fabs(ISH - ISL);      /* alternative reading G2 (A); never the default */
+    if (g_g2_variant == 0) ISt = fabs(ISH - ISL);   /* alternative reading G2 (A); never the default */
+    if (g_g2_variant == 2) ISt = IS4[3];            /* negative control of oracle/readings_table.py: fourth-derivative part only */
     double aH = 1.0 + pow(ISt / (ISH + eps), p->geno_r), aL = 1.0 + pow(ISt / (ISL + eps), p->geno_r);
     double alpha = 2.0 * aH / (aH + aL);
     chi = tanh(p->geno_C * alpha) / tanh(p->geno_C);

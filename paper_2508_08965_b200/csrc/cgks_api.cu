@@ -193,8 +193,11 @@ static int create_impl(cgks_ctx** out, int ni, int nj, int nkg, int nk, int kofs
   do {
     if (cudaMemsetAsync(c->d_flags, 0, 64, c->stream) != cudaSuccess) { bail(CGKS_ECUDA, "cudaMemsetAsync failed"); break; }
     const unsigned gridg = (unsigned)((n + TPB - 1) / TPB);
-    // pass 1: validity + uniform-Cartesian detection (no metric storage)
-    geometry_kernel<<<gridg, TPB, 0, c->stream>>>(ni, nj, nkg, nk, kofs, d_nodes, nullptr, c->d_flags); c->launches++;
+    // pass 1: validity + uniform-Cartesian detection (no metric storage), over the WHOLE global mesh also for a sub-domain:
+    // whether the mesh is uniform Cartesian (constant metrics, CART kernels) is a property of the mesh, not of the slab, so
+    // every rank of a decomposition takes the same code path and a cell's update is bit-identical whichever context holds it
+    const unsigned gridall = (unsigned)(((long)ni * nj * nkg + TPB - 1) / TPB);
+    geometry_kernel<<<gridall, TPB, 0, c->stream>>>(ni, nj, nkg, nkg, 0, d_nodes, nullptr, c->d_flags); c->launches++;
     int flags[4] = { 0, 0, 0, 0 };
     cudaError_t e = cudaMemcpyAsync(flags, c->d_flags, sizeof flags, cudaMemcpyDeviceToHost, c->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);

@@ -61,6 +61,31 @@ def test_subdomains_equal_the_single_domain_bit_for_bit(name, n, world):
     assert dts == dts_ref
     for a, b in zip(got, ref):
         assert np.array_equal(a, b)
+    # ... and the decomposed run against the ORACLE (not only against the GPU itself), stepping the oracle with the same dts;
+    # the bar is north_star's 1e-10 per step
+    orc, _ = parity.run_oracle(w, 5, dts=dts)
+    errs = parity.field_errors(got, orc, w["nodes"], w["Q"])
+    worst = max(errs, key=errs.get)
+    assert errs[worst] <= 5 * 1e-10, (worst, errs[worst])
+
+
+def test_mesh_type_is_a_property_of_the_mesh_not_of_the_slab():
+    """A mesh that is uniform Cartesian everywhere except in cell planes 8..10: the sub-domain that holds planes 16, 17, 0..7
+    sees only uniform cells, yet it must run the general-mesh kernels like its neighbours and like the single-domain context
+    (cgks_create_slab decides on the WHOLE node array), or its cells would not be bit-identical."""
+    n = 18
+    w = parity.build_case("tgv", n, 1)
+    nodes = w["nodes"].copy()
+    h = 2.0 * np.pi / n
+    bump = 0.1 * h * np.sin(2.0 * np.pi * np.arange(n + 1) / n)             # periodic in i: nodes 0 and n unmoved
+    for k in (9, 10):
+        nodes[0, k] += bump[None, :]
+    w["nodes"] = nodes
+    ref, dts_ref = _single(w, 2)
+    got, dts = _slabs(w, 2, 3)
+    assert dts == dts_ref
+    for a, b in zip(got, ref):
+        assert np.array_equal(a, b)
 
 
 def test_subdomain_with_its_own_slab_pipeline():
@@ -98,3 +123,24 @@ def test_slab_solver_world_of_one_and_error_codes():
     full.close()
     with pytest.raises(binding.CgksError):
         binding.Solver(w["nodes"], binding.make_params(**w["params"]), slab=(0, 1))          # fewer than 2 owned planes
+
+
+def test_bench_slab_mode_on_one_rank():
+    """bench.py --parallel slab at N = 1 (the code path the driver's scaling run uses): one JSON line with the contract's keys,
+    the roofline on its fixed FP64 basis, an end-to-end number with its copies declared."""
+    import json
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    r = subprocess.run([sys.executable, "bench.py", "--n", "64", "--steps", "2", "--warmup", "3", "--gpus", "1", "--parallel", "slab",
+                        "--no-cpu-baseline"], cwd=root, capture_output=True, text=True, timeout=900)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [json.loads(l) for l in r.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1
+    d = lines[0]
+    assert d["value"] > 0 and d["n_gpus"] == 1 and d["dtype"] == "f64" and d["gpu_launches"] > 0
+    assert "slab decomposition" in d["config"]["parallelism"]
+    assert d["roofline"]["bound"] == "alu" and 0 < d["roofline"]["frac"] < 1 and "frac_as_built_bytes" in d["roofline"]
+    assert d["roofline"]["whole_step"]["compulsory_bytes_per_cell"] == 4000.0
+    assert d["e2e"]["value"] > 0 and d["e2e"]["h2d_bytes_per_step"] > 0
