@@ -56,6 +56,22 @@ RECON_FP64_INSTR_PER_CELLVAR = 1516.0
 COMPULSORY_BYTES_PER_CELL = 4000.0            # 500 doubles per cell and step, state in / state out only
 DRAM_BYTES_PER_CELL_NCU = 21970.0             # profiles/r02k_dram_384.csv: 1.244 TB per 384^3 step
 FP64_PEAK_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12      # SMs x FP64 FMA lanes x 2 x max SM clock = 37.2
+# Per-kernel constants by mesh type.  "cart": the uniform-Cartesian kernels (sweep_kernel<1,..>, recon_kernel<1,..>), capture
+# profiles/r02k_final.md.  "general": the general-mesh kernels (sweep_kernel<0,..>, recon_kernel<0,..>: metric loads, J0 / J0^-1
+# transforms, face frames built from the stored vector areas), capture profiles/r03a_curvilinear.md.
+KERNEL_CONSTANTS = {
+    "cart": {"sweep_flops": (SWEEP_FLOPS_STAGE1, SWEEP_FLOPS_STAGE2), "sweep_instr": SWEEP_FP64_INSTR, "sweep_bytes": SWEEP_BYTES_ALG,
+             "sweep_traffic": SWEEP_TRAFFIC, "pipe_active": SWEEP_FP64_PIPE_ACTIVE_NCU, "recon_flops": RECON_FLOPS_PER_CELLVAR,
+             "recon_instr": RECON_FP64_INSTR_PER_CELLVAR, "recon_bytes_cell": 4480.0, "dram_bytes_per_cell": DRAM_BYTES_PER_CELL_NCU,
+             "compulsory_bytes_per_cell": COMPULSORY_BYTES_PER_CELL, "capture": "profiles/r02k_final.md"},
+    # general meshes, per EXECUTED point like the Cartesian figures (per useful point at 128^3: 2963 / 2924 / 2924 flops in stage 1,
+    # 2616 / 2578 / 2579 in stage 2, divided by 1.0625 for AX = 0 and 1.047 for AX = 1, 2); reconstruction 1030 DFMA + 307 DMUL + 449 DADD
+    "general": {"sweep_flops": (2791.0, 2462.0), "sweep_instr": (1758.0, 1544.0),
+                "sweep_bytes": (SWEEP_BYTES_ALG[0] + 12.7, SWEEP_BYTES_ALG[1] + 12.7),      # + the face's vector area and tangent (48 B per face) and the cell volume
+                "sweep_traffic": (571.4, 505.8), "pipe_active": (0.520, 0.602), "recon_flops": 2816.0, "recon_instr": 1786.0,
+                "recon_bytes_cell": 4480.0 + 144.0, "dram_bytes_per_cell": 24524.0,
+                "compulsory_bytes_per_cell": COMPULSORY_BYTES_PER_CELL + 2 * 296.0, "capture": "profiles/r03a_curvilinear.md"},
+}
 
 
 def parse():
@@ -64,6 +80,9 @@ def parse():
     ap.add_argument("--steps", type=int, default=4)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--n", "--size", dest="n", type=int, default=384, help="cells per direction (default: the 384^3 headline config)")
+    ap.add_argument("--workload", default="iso_sup", choices=["iso_sup", "tgv_curv"],
+                    help="iso_sup: the headline config (BASELINE.json configs[4], Cartesian); tgv_curv: Taylor-Green vortex on the "
+                         "non-orthogonal curvilinear mesh of configs[2] (general-mesh kernels; use --n 256)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -175,11 +194,24 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=dev)
     use_slab = args.parallel == "slab"
     n = args.n
-    k0 = 8.0 if n >= 128 else 2.0
-    prm = inputs.iso_params(1.0, k0=k0)
-    nodes = torch.from_numpy(inputs.cartesian_nodes(n)).to(dev)
-    # replicas: one seed per rank (independent problems); slab: every rank builds the one global field and keeps its slab
-    Q = inputs.iso_turbulence(n, 5 + (0 if use_slab else rank), 1.0, k0, device=dev).contiguous()
+    curv = args.workload == "tgv_curv"
+    if curv:
+        if use_slab:
+            raise SystemExit("bench.py: --workload tgv_curv runs on a whole-mesh context (no --parallel slab)")
+        prm = inputs.tgv_params()
+        nodes_np = inputs.curvilinear_nodes(n)
+        Q = torch.from_numpy(inputs.taylor_green(nodes_np)).to(dev).contiguous()
+        nodes = torch.from_numpy(nodes_np).to(dev)
+        del nodes_np
+        workload_name = "tgv_curv: Taylor-Green vortex Re=1600 Ma=0.1 on the non-orthogonal periodic curvilinear %d^3 mesh (BASELINE.json configs[2] at %d^3)" % (n, n)
+    else:
+        k0 = 8.0 if n >= 128 else 2.0
+        prm = inputs.iso_params(1.0, k0=k0)
+        nodes = torch.from_numpy(inputs.cartesian_nodes(n)).to(dev)
+        # replicas: one seed per rank (independent problems); slab: every rank builds the one global field and keeps its slab
+        Q = inputs.iso_turbulence(n, 5 + (0 if use_slab else rank), 1.0, k0, device=dev).contiguous()
+        workload_name = "iso_sup: supersonic isotropic turbulence Ma_t=1.0, periodic Cartesian %d^3 (BASELINE.json configs[4])" % n
+    K = KERNEL_CONSTANTS["general" if curv else "cart"]
     params = binding.make_params(**prm, nonlinear=1)
     if use_slab:
         k_lo, nk_own = slab.partition(n, world)[rank]
@@ -287,18 +319,18 @@ def run_ours(args):
         # summed over the launches of the profiled steps the useful points are 12 per cell per stage (the extra first face of
         # every line of a sweep is redundant work and not counted)
         pts_per_stage = 12 * cells_rank
-        flops = (SWEEP_FLOPS_STAGE1 + SWEEP_FLOPS_STAGE2) * pts_per_stage * psteps
+        flops = sum(K["sweep_flops"]) * pts_per_stage * psteps
         ach = flops / (fms * 1e-3) / 1e12
         pts_per_launch = 2 * pts_per_stage * psteps / fnl
         sm_mhz = clocks.get("sm_mhz") or 1965.0
         # reconstruction: HBM-bound, 640 B read + 3840 B written per cell (+ the two extra planes of every slab)
         nchunks = 1 if solver_slab(solver) >= (nk_own + 4 if use_slab else n) else math.ceil((nk_own if use_slab else n) / solver_slab(solver))
         planes = (nk_own if use_slab else n) + (2 * nchunks if (use_slab or nchunks > 1) else 0)
-        recon_bytes = 2 * psteps * 4480.0 * planes * n * n
+        recon_bytes = 2 * psteps * K["recon_bytes_cell"] * planes * n * n
         hbm_peak = measured_hbm_peak()
         # which roof binds (north_star: "the slower of bytes at HBM bandwidth and flops at FP64 peak"): the kernel's arithmetic
         # intensity, executed flops / algorithmic bytes, against the machine balance
-        alg_bytes_launch = 0.5 * sum(SWEEP_BYTES_ALG) * pts_per_launch
+        alg_bytes_launch = 0.5 * sum(K["sweep_bytes"]) * pts_per_launch
         gbs = alg_bytes_launch / (fms / fnl * 1e-3) / 1e9
         t_hbm = gbs / hbm_peak[0]; t_alu = ach / FP64_PEAK_NOMINAL_TFLOPS
         # `frac` has ONE basis, the same in every round: the FP64 roof on the flops this kernel executes ("the plain
@@ -313,24 +345,24 @@ def run_ours(args):
                               "bytes the pipeline AS BUILT moves per point (incl. 320 B of reads of the intermediate pv buffer) / time / HBM peak "
                               "(%.1f GB/s, %s): a utilisation figure of this design's own traffic, not a roofline fraction" % (hbm_peak[0], hbm_peak[1]),
                 "hbm_on_pipeline_bytes": {"achieved": gbs, "peak": hbm_peak[0], "unit": "GB/s", "frac_as_built_bytes": t_hbm, "peak_source": hbm_peak[1],
-                                          "bytes_per_point": list(SWEEP_BYTES_ALG), "of_which_pv_reads": 320.0},
+                                          "bytes_per_point": list(K["sweep_bytes"]), "of_which_pv_reads": 320.0},
                 "alu": {"achieved": ach, "peak": FP64_PEAK_NOMINAL_TFLOPS, "unit": "TFLOP/s", "frac": t_alu,
                         "frac_at_measured_clock": ach / (FP64_PEAK_NOMINAL_TFLOPS * sm_mhz / 1965.0)},
-                "flops_per_point_executed": [SWEEP_FLOPS_STAGE1, SWEEP_FLOPS_STAGE2],
+                "flops_per_point_executed": list(K["sweep_flops"]), "constants_from": K["capture"],
                 "flops_per_point_oracle_counted": FLUX_FLOPS_ORACLE,
-                "achieved_with_oracle_count": ach * 2.0 * FLUX_FLOPS_ORACLE / (SWEEP_FLOPS_STAGE1 + SWEEP_FLOPS_STAGE2),
-                "frac_with_r01_flop_count": ach * sum(FLUX_FLOPS_R01) / (SWEEP_FLOPS_STAGE1 + SWEEP_FLOPS_STAGE2) / FP64_PEAK_NOMINAL_TFLOPS,
-                "fp64_pipe_active_ncu": list(SWEEP_FP64_PIPE_ACTIVE_NCU),
+                "achieved_with_oracle_count": ach * 2.0 * FLUX_FLOPS_ORACLE / sum(K["sweep_flops"]),
+                "frac_with_r01_flop_count": ach * sum(FLUX_FLOPS_R01) / sum(K["sweep_flops"]) / FP64_PEAK_NOMINAL_TFLOPS,
+                "fp64_pipe_active_ncu": list(K["pipe_active"]),
                 "flops_note": "achieved = flops EXECUTED by this kernel's own (leanest known) formulation per useful point / time, so a leaner "
                               "formulation lowers it at equal pipe utilisation (round 1's flux kernel executed 42 % more flops per point for "
                               "the same result); 36 % of its FP64 instructions are DMUL/DADD, which occupy an FMA slot for one flop: at 100 % "
                               "pipe activity this instruction mix reaches 0.79 of the FMA peak; the peak assumes the maximum SM clock, the "
                               "box runs below it under its 1 kW power cap (frac_at_measured_clock uses the sampled clock); the CPU oracle's "
                               "term-by-term evaluation needs 7x the arithmetic, so its count would give a fraction above 1 (DESIGN.md 7.2)",
-                "traffic": 0.5 * sum(SWEEP_TRAFFIC) * pts_per_launch,
+                "traffic": 0.5 * sum(K["sweep_traffic"]) * pts_per_launch,
                 "pipeline_bytes": alg_bytes_launch,
                 "traffic_note": "bytes per average launch = ncu dram bytes per point (profiles/r02k_final.md) x points per launch; "
-                                "pipeline bytes per point as built %.0f (stage 1) / %.0f (stage 2), 320 of them reads of pv" % SWEEP_BYTES_ALG,
+                                "pipeline bytes per point as built %.0f (stage 1) / %.0f (stage 2), 320 of them reads of pv" % tuple(K["sweep_bytes"]),
                 "peak_source": "HBM: " + hbm_peak[1] + "; FP64: derived, 148 SMs x 64 FP64 FMA lanes x 2 x 1.965 GHz (DESIGN.md section 7), "
                                "MEASURED_PEAKS.json has no FP64 entry",
                 "peak_dfma_microbench": peak_meas, "frac_of_dfma_microbench": (ach / peak_meas) if peak_meas else None,
@@ -338,21 +370,26 @@ def run_ours(args):
                 "share_of_step": fms / (pms if pms > 0 else 1.0),
                 "kernel_ms_per_step": {k: v[0] / psteps for k, v in kms.items()},
                 "profiled_steps": psteps, "profiled_ms_per_step": pms / psteps,
-                "whole_step": whole_step(pms / psteps, cells_rank, hbm_peak[0], sm_mhz),
+                "whole_step": whole_step(K, pms / psteps, cells_rank, hbm_peak[0], sm_mhz),
                 "other_kernels": {"recon_kernel": {
                     "bound": "hbm", "achieved": recon_bytes / (rms * 1e-3) / 1e9 if rms > 0 else None, "peak": hbm_peak[0], "unit": "GB/s",
                     "frac": (recon_bytes / (rms * 1e-3) / 1e9 / hbm_peak[0]) if rms > 0 else None, "peak_source": hbm_peak[1],
-                    "algorithmic_bytes_per_cell": 4480.0, "avg_launch_ms": rms / rnl if rnl else None, "launches": rnl,
+                    "algorithmic_bytes_per_cell": K["recon_bytes_cell"], "avg_launch_ms": rms / rnl if rnl else None, "launches": rnl,
                     "share_of_step": rms / (pms if pms > 0 else 1.0)}}}
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
             "ms_per_step": ms_max / args.steps, "higher_is_better": True, "scaling": "strong" if use_slab and world > 1 else "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": "iso_sup: supersonic isotropic turbulence Ma_t=1.0, periodic Cartesian %d^3 (BASELINE.json configs[4])" % n,
+            "config": {"workload": workload_name,
                        "cells": n ** 3, "nonlinear": 1, "cfl": 0.5,
                        "parallelism": ("slab decomposition along k, %d ranks" % world) if use_slab else ("replicas only" if world > 1 else "single GPU"),
                        "l2": "inputs larger than L2 (state %.1f GB per buffer)" % (80 * cells_rank * 8 / 1e9),
                        "slab_depth": solver_slab(solver), "chi_below_0.99_fraction": chi_frac},
             "clocks": clocks, "gpu_launches": launches, "e2e": e2e, "roofline": roof}
+    if e2e is not None and world == 1 and not use_slab:
+        # the full 80-dof state through the same host call, measured (not estimated) on a mesh whose state fits a pinned buffer
+        solver.close(); del solver
+        torch.cuda.empty_cache()
+        e2e["full_state"] = full_state_e2e(dev, max(args.steps, 2))
     if rank == 0:
         if not args.no_cpu_baseline and world == 1:
             line["cpu_baseline"] = cpu_baseline()
@@ -361,22 +398,23 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
-def whole_step(ms_step, cells, hbm_gbs, sm_mhz):
+def whole_step(K, ms_step, cells, hbm_gbs, sm_mhz):
     """The whole S2O4 step against its two floors: compulsory HBM bytes (state in / state out only: stage 1
     reads 80 and writes 80 + 90 doubles per cell, stage 2 reads 80 + 90 and writes 80 -> 500 doubles = 4.0 kB per cell) and
     executed FP64 work.  Everything a reader needs to recompute the fractions is in the object."""
     t = ms_step * 1e-3
-    flops_cell = 12.0 * (SWEEP_FLOPS_STAGE1 + SWEEP_FLOPS_STAGE2) + 2.0 * 5.0 * RECON_FLOPS_PER_CELLVAR
-    instr_cell = 12.0 * sum(SWEEP_FP64_INSTR) + 2.0 * 5.0 * RECON_FP64_INSTR_PER_CELLVAR
+    flops_cell = 12.0 * sum(K["sweep_flops"]) + 2.0 * 5.0 * K["recon_flops"]
+    instr_cell = 12.0 * sum(K["sweep_instr"]) + 2.0 * 5.0 * K["recon_instr"]
     # one FP64 instruction per lane per cycle: 148 SMs x 64 lanes at the sampled clock
     instr_rate_peak = 148 * 64 * sm_mhz * 1e6
-    built = 2 * 4480.0 + 12.0 * sum(SWEEP_BYTES_ALG)
-    return {"compulsory_bytes_per_cell": COMPULSORY_BYTES_PER_CELL,
+    built = 2 * K["recon_bytes_cell"] + 12.0 * sum(K["sweep_bytes"])
+    comp = K["compulsory_bytes_per_cell"]; dram = K["dram_bytes_per_cell"]
+    return {"compulsory_bytes_per_cell": comp,
             "pipeline_bytes_per_cell": built,
-            "dram_bytes_per_cell_ncu": DRAM_BYTES_PER_CELL_NCU,
-            "traffic_ratio": DRAM_BYTES_PER_CELL_NCU / COMPULSORY_BYTES_PER_CELL,
-            "hbm_floor_ms_compulsory": COMPULSORY_BYTES_PER_CELL * cells / hbm_gbs / 1e6,
-            "frac_of_compulsory_hbm_floor": COMPULSORY_BYTES_PER_CELL * cells / hbm_gbs / 1e9 / t,
+            "dram_bytes_per_cell_ncu": dram,
+            "traffic_ratio": (dram / comp) if dram else None,
+            "hbm_floor_ms_compulsory": comp * cells / hbm_gbs / 1e6,
+            "frac_of_compulsory_hbm_floor": comp * cells / hbm_gbs / 1e9 / t,
             "hbm_floor_ms_as_built": built * cells / hbm_gbs / 1e6,
             "frac_as_built_bytes": built * cells / hbm_gbs / 1e9 / t,
             "fp64_flops_per_cell_executed": flops_cell,
@@ -386,6 +424,35 @@ def whole_step(ms_step, cells, hbm_gbs, sm_mhz):
             "fp64_pipe_busy_at_sampled_clock": instr_cell * cells / t / instr_rate_peak,
             "note": "dram_bytes_per_cell_ncu and the instruction counts are constants of the committed ncu capture named in bench.py; "
                     "traffic_ratio = measured DRAM bytes / compulsory bytes (1.0 = no intermediate traffic at all)"}
+
+
+def full_state_e2e(dev, steps, n=128):
+    """cgks_run_host with ALL 80 fields per cell (Q, G, D) shipped host->device from pinned memory, one S2O4 step, all 80 shipped
+    back: the warm-restart counterpart of the Q-only end-to-end leg, on the 128^3 supersonic-turbulence mesh (the 384^3 state
+    is 36 GB each way and would time the PCIe link only)."""
+    import torch
+    from paper_2508_08965_b200 import binding, inputs
+    prm = inputs.iso_params(1.0, k0=8.0)
+    nodes = torch.from_numpy(inputs.cartesian_nodes(n)).to(dev)
+    Q = inputs.iso_turbulence(n, 5, 1.0, 8.0, device=dev).contiguous()
+    sol = binding.Solver(nodes, binding.make_params(**prm, nonlinear=1), device=dev)
+    sol.set_state(Q)
+    sol.step(sol.compute_dt(0.5))                           # a developed set of derivative dof
+    host_in = [torch.empty(t.shape, dtype=torch.float64, pin_memory=True) for t in sol.get_state()]
+    for h, t in zip(host_in, sol.get_state()):
+        h.copy_(t)
+    host_out = [torch.empty(h.shape, dtype=torch.float64, pin_memory=True) for h in host_in]
+    torch.cuda.synchronize(dev)
+    sol.run_host(*host_in, 0.5, 1, *host_out)               # warm
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        sol.run_host(*host_in, 0.5, 1, *host_out)           # synchronises inside (cgks_status)
+    dt = time.perf_counter() - t0
+    sol.close()
+    nb = int(sum(h.numel() for h in host_in) * 8)
+    return {"value": n ** 3 * steps / dt, "unit": UNIT, "cells": n ** 3, "h2d_bytes_per_step": nb, "d2h_bytes_per_step": nb,
+            "ms_per_step": 1e3 * dt / steps,
+            "note": "iso_sup at %d^3: Q, G and D (80 doubles per cell) host->device from pinned memory, one full S2O4 step, all 80 back" % n}
 
 
 def measured_hbm_peak():
