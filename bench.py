@@ -69,7 +69,7 @@ KERNEL_CONSTANTS = {
     "general": {"sweep_flops": (2791.0, 2462.0), "sweep_instr": (1758.0, 1544.0),
                 "sweep_bytes": (SWEEP_BYTES_ALG[0] + 12.7, SWEEP_BYTES_ALG[1] + 12.7),      # + the face's vector area and tangent (48 B per face) and the cell volume
                 "sweep_traffic": (571.4, 505.8), "pipe_active": (0.520, 0.602), "recon_flops": 2816.0, "recon_instr": 1786.0,
-                "recon_bytes_cell": 4480.0 + 144.0, "dram_bytes_per_cell": 24524.0,
+                "recon_bytes_cell": 4480.0 + 144.0, "dram_bytes_per_cell": 23560.0,      # after r03b (recon reads 16.9 instead of 25.0 GB per launch at 256^3)
                 "compulsory_bytes_per_cell": COMPULSORY_BYTES_PER_CELL + 2 * 296.0, "capture": "profiles/r03a_curvilinear.md"},
 }
 

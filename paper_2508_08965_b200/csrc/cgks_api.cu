@@ -388,7 +388,7 @@ static void run_stage(cgks_ctx* c, int stage, double dt) {
   sl.stride_pv = (long)c->slots_pv * m.plane; sl.stride_fx = (long)c->slots_fx * m.plane;
   auto recon = [&](int kA, int cnt) {
     const long nt = (long)cnt * m.plane;
-    dim3 grid((unsigned)((nt + TPB - 1) / TPB), 5);
+    const dim3 grid = recon_grid<CART>(nt, TPB);
     Timed t(c, KC_RECON);
     if (rp.nonlinear) recon_kernel<CART, false, true><<<grid, TPB, 0, c->stream>>>(m, sl, Win, c->pv, c->chi, rp, kA, nt, c->d_flags + 3);
     else recon_kernel<CART, false, false><<<grid, TPB, 0, c->stream>>>(m, sl, Win, c->pv, c->chi, rp, kA, nt, c->d_flags + 3);
@@ -493,7 +493,7 @@ extern "C" int cgks_debug_stage(cgks_ctx* c, double dt, double* d_pv, double* d_
   Slab sl; sl.kbase = 0; sl.slots_pv = c->slots_pv; sl.slots_fx = c->slots_fx;
   sl.stride_pv = (long)c->slots_pv * m.plane; sl.stride_fx = (long)c->slots_fx * m.plane;
   const long nt = m.n;
-  dim3 grid((unsigned)((nt + TPB - 1) / TPB), 5);
+  const dim3 grid = m.cart ? recon_grid<true>(nt, TPB) : recon_grid<false>(nt, TPB);
   const double* Win = c->W[c->cur];
   if (m.cart) { if (rp.nonlinear) recon_kernel<true, false, true><<<grid, TPB, 0, c->stream>>>(m, sl, Win, c->pv, c->chi, rp, 0, nt, c->d_flags + 3); else recon_kernel<true, false, false><<<grid, TPB, 0, c->stream>>>(m, sl, Win, c->pv, c->chi, rp, 0, nt, c->d_flags + 3); }
   else { if (rp.nonlinear) recon_kernel<false, false, true><<<grid, TPB, 0, c->stream>>>(m, sl, Win, c->pv, c->chi, rp, 0, nt, c->d_flags + 3); else recon_kernel<false, false, false><<<grid, TPB, 0, c->stream>>>(m, sl, Win, c->pv, c->chi, rp, 0, nt, c->d_flags + 3); }
@@ -524,8 +524,8 @@ static void run_diagnostics(cgks_ctx* c, double* d_acc) {
     sl.kbase = k0;
     const long nt = (long)cnt * m.plane;
     const unsigned nb = (unsigned)((nt + TPB - 1) / TPB);
-    { Timed t(c, KC_OTHER); if (rp.nonlinear) recon_kernel<CART, true, true><<<dim3(nb, 5), TPB, 0, c->stream>>>(m, sl, Win, c->pv, nullptr, rp, k0, nt, c->d_flags + 3);
-      else recon_kernel<CART, true, false><<<dim3(nb, 5), TPB, 0, c->stream>>>(m, sl, Win, c->pv, nullptr, rp, k0, nt, c->d_flags + 3); }
+    { Timed t(c, KC_OTHER); if (rp.nonlinear) recon_kernel<CART, true, true><<<recon_grid<CART>(nt, TPB), TPB, 0, c->stream>>>(m, sl, Win, c->pv, nullptr, rp, k0, nt, c->d_flags + 3);
+      else recon_kernel<CART, true, false><<<recon_grid<CART>(nt, TPB), TPB, 0, c->stream>>>(m, sl, Win, c->pv, nullptr, rp, k0, nt, c->d_flags + 3); }
     { Timed t(c, KC_OTHER); diag_kernel<CART><<<nb, TPB, 0, c->stream>>>(m, sl, Win, c->pv, dp, k0, nt, scratch); }
     { Timed t(c, KC_OTHER); diag_reduce_kernel<<<1, 256, 0, c->stream>>>(scratch, (long)nb, d_acc); }
   }

@@ -95,13 +95,24 @@ __device__ __forceinline__ void recon_gather_axis(const ReconCell<CART>& rc, con
 // (pv planes 0..7, used by the diagnostics of PAPER.md:428-454).
 // NL: the GENO blend is compiled in (nonlinear = 1, the paper's default) or out (linear scheme), so that the thread is one block of
 // straight-line code either way.
+// launch grid of recon_kernel over nthreads cells with blocks of tpb threads (see the index computation in the kernel)
+template <bool CART>
+inline dim3 recon_grid(long nthreads, int tpb) {
+  const unsigned tiles = (unsigned)((nthreads + tpb - 1) / tpb);
+  return CART ? dim3(tiles, 5) : dim3(tiles * 5u, 1);
+}
+
 template <bool CART, bool VOLUME = false, bool NL = true>
 __global__ void __launch_bounds__(128, 3) recon_kernel(Mesh m, Slab sl, const double* __restrict__ W, double* __restrict__ pv,
                                                     double* __restrict__ chi_out, ReconPrm rp, int kA, long nthreads,
                                                     int* __restrict__ flag) {
-  const long t = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  // Cartesian: grid (tiles, 5), v = blockIdx.y.  General meshes: grid (5 tiles), the five variable-blocks of a tile ADJACENT in launch
+  // order (v = blockIdx.x % 5), so that the 18 doubles of J0 / J0^-1 per cell, which all five read, come from DRAM once and from L2
+  // four times (with v = blockIdx.y the five readers run a whole grid row apart and every read misses: profiles/r03a_curvilinear.md)
+  const unsigned tile = CART ? blockIdx.x : blockIdx.x / 5u;
+  const int v = CART ? (int)blockIdx.y : (int)(blockIdx.x - 5u * tile);
+  const long t = (long)tile * blockDim.x + threadIdx.x;
   if (t >= nthreads) return;
-  const int v = blockIdx.y;
   const CellIdx x = cell_of(m, t, kA);
   const long n = m.n;
   if (v == 0) {      // physical admissibility of the incoming cell average (reported by cgks_status / cgks_compute_dt)

@@ -133,6 +133,10 @@ def test_bench_slab_mode_on_one_rank():
     import subprocess
     import sys
     root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    # this process may still hold most of the device in torch's caching allocator (the 384^3 cases): give it back to the driver,
+    # the child process allocates its own workspace
+    import gc
+    gc.collect(); torch.cuda.empty_cache()
     r = subprocess.run([sys.executable, "bench.py", "--n", "64", "--steps", "2", "--warmup", "3", "--gpus", "1", "--parallel", "slab",
                         "--no-cpu-baseline"], cwd=root, capture_output=True, text=True, timeout=900)
     assert r.returncode == 0, r.stderr[-2000:]
