@@ -545,7 +545,7 @@ def _block_nodes(nodes, lo, B):
 
 
 @pytest.mark.parametrize("case", ["iso_sup_384_after_100", "iso_sub_128_after_100", "tgv_sup_128_shocked", "tgv_curv_64_after_100",
-                                  "iso_sup_64_rough_after_50", "tgv_sup_320_shocked"])
+                                  "tgv_64_after_100", "iso_sup_64_rough_after_50", "tgv_sup_320_shocked"])
 def test_restart_parity(case):
     """Multi-step and shock-active states at sizes the oracle cannot run as a whole (north_star: 100 steps on all five
     configs; Ma = 1.25 vortex once shocklets have formed): the library runs the steps on the full
@@ -572,16 +572,18 @@ def test_restart_parity(case):
         budget = 0
     elif case in ("tgv_sup_128_shocked", "tgv_sup_320_shocked"):
         n = 128 if "128" in case else 320               # the two mesh sizes of the paper's Ma = 1.25 runs
-        if n == 320 and not os.environ.get("CGKS_LONG_TESTS"):
-            pytest.skip("about 1400 steps at 320^3 (5 GPU-minutes): set CGKS_LONG_TESTS=1; result recorded in DESIGN.md 9b")
+        # the paper's own mesh for this run: about 1400 steps at 320^3, 5 GPU-minutes.  Runs by default on a
+        # device that can hold it, so that the driver's GPU run sees the paper's size; CGKS_SKIP_LONG_TESTS=1 opts out
+        if n == 320 and os.environ.get("CGKS_SKIP_LONG_TESTS"):
+            pytest.skip("CGKS_SKIP_LONG_TESTS is set")
         if n == 320 and free < 150e9:
             pytest.skip("needs a 180 GB device")
         steps, B, nb = 0, 24, 6
         w = inputs.workload("tgv_sup", n); prm = w["params"]; nonlinear = 1; nodes = w["nodes"]; Q = w["Q"]
         budget = 0 if n == 128 else int(free - 30e9)
-    elif case == "tgv_curv_64_after_100":
+    elif case in ("tgv_curv_64_after_100", "tgv_64_after_100"):      # BASELINE.json configs[2] and configs[1] at full size
         n, steps, B, nb = 64, 100, 24, 4
-        w = inputs.workload("tgv_curv", n); prm = w["params"]; nonlinear = 1; nodes = w["nodes"]; Q = w["Q"]
+        w = inputs.workload("tgv_curv" if "curv" in case else "tgv", n); prm = w["params"]; nonlinear = 1; nodes = w["nodes"]; Q = w["Q"]
         budget = 0
     else:
         n, steps, B, nb = 64, 50, 24, 4
