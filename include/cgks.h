@@ -106,9 +106,9 @@ const char* cgks_static_last_error(void);
 
 /* One two-stage fourth-order step of size dt.  Asynchronous.
    Per stage: one reconstruction kernel (Eq. 11-19), then one sweep kernel per face direction that computes the gas-kinetic
-   flux at the face Gauss points (Eq. 1-7) and accumulates Eq. 8-10 and the S2O4 combine into the state buffers.  With
-   CGKS_PIPELINE=split in the environment at cgks_create time the stage instead runs the three-kernel pipeline of the first
-   rounds (flux -> face-flux buffer -> update): same results to round-off, kept for A/B timing. */
+   flux at the face Gauss points (Eq. 1-7) and accumulates Eq. 8-10 and the S2O4 combine into the state buffers.  (The
+   three-kernel pipeline of the first rounds, flux -> face-flux buffer -> update, exists only in the test-only A/B build
+   libcgks_ab.so and as the flux tap of cgks_debug_stage; nothing selects it at run time.) */
 int cgks_step(cgks_ctx*, double dt);
 
 /* One stage of the step (1: state n -> stage state; 2: stage state -> state n+1); cgks_step(dt) is

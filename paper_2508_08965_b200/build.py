@@ -37,5 +37,21 @@ def build(force=False, verbose=False):
     return LIB
 
 
+LIB_AB = os.path.join(HERE, "libcgks_ab.so")
+
+
+def build_ab(force=False):
+    """TEST-ONLY A/B library: the same sources with -DCGKS_AB_SPLIT_PIPELINE, i.e. every stage runs the three-kernel pipeline of
+    rounds 1-2 (flux -> face-flux buffer -> update) instead of the sweep kernels.  tests/test_gpu_parity.py loads it to compare
+    the two pipelines; the product (binding.py, bench.py) never does."""
+    generate(False)
+    deps = [os.path.join(CSRC, f) for f in SOURCES + HEADERS] + [os.path.join(HERE, "..", "include", "cgks.h")]
+    if not force and os.path.exists(LIB_AB) and all(not _newer(d, LIB_AB) for d in deps):
+        return LIB_AB
+    nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+    subprocess.check_call([nvcc] + NVCC_FLAGS + ["-DCGKS_AB_SPLIT_PIPELINE", "-o", LIB_AB] + [os.path.join(CSRC, s) for s in SOURCES])
+    return LIB_AB
+
+
 if __name__ == "__main__":
     print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))

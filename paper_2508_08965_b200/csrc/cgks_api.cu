@@ -66,7 +66,11 @@ static int cuda_fail(cgks_ctx* c, cudaError_t e, const char* where) {
 }
 #define CK(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail(c, e_, #call); } while (0)
 
+#ifdef CGKS_AB_SPLIT_PIPELINE
+extern "C" const char* cgks_version(void) { return "cgks-b200 0.1 (sm_100a, fp64) TEST BUILD: three-kernel pipeline"; }
+#else
 extern "C" const char* cgks_version(void) { return "cgks-b200 0.1 (sm_100a, fp64)"; }
+#endif
 // message of the last failed cgks_create of the calling thread (there is no context to hold it)
 static thread_local std::string g_create_err;
 extern "C" const char* cgks_last_create_error(void) { return g_create_err.c_str(); }
@@ -74,8 +78,15 @@ extern "C" const char* cgks_last_error(const cgks_ctx* c) { return c ? c->err.c_
 extern "C" long cgks_launch_count(const cgks_ctx* c) { return c ? c->launches : 0; }
 extern "C" int cgks_slab_depth(const cgks_ctx* c) { return c ? c->S : 0; }
 
-// CGKS_PIPELINE=split in the environment selects the three-kernel pipeline of rounds 1-2 (A/B timing, test taps)
-static bool pipeline_split() { const char* e = getenv("CGKS_PIPELINE"); return e && strcmp(e, "split") == 0; }
+// The product library (libcgks.so) has ONE pipeline: the sweep kernels.  The three-kernel pipeline of rounds 1-2 (flux -> face-flux
+// buffer -> update) survives only (a) as the flux tap of cgks_debug_stage and (b) in the test-only A/B build libcgks_ab.so
+// (build.build_ab(): this file compiled with -DCGKS_AB_SPLIT_PIPELINE), which tests/ load to compare the two.  No environment
+// variable and no run-time dispatch selects it.
+#ifdef CGKS_AB_SPLIT_PIPELINE
+static constexpr bool pipeline_split() { return true; }
+#else
+static constexpr bool pipeline_split() { return false; }
+#endif
 
 static size_t fixed_bytes(long n, bool with_metrics) {
   size_t b = 3 * state_bytes(n) + align_up((size_t)5 * n * 8) + align_up(64);
@@ -226,7 +237,7 @@ static int create_impl(cgks_ctx** out, int ni, int nj, int nkg, int nk, int kofs
     }
     // slab buffers from what is left.  Sweep pipeline (default): reconstructed face values (pv) only; the face-flux buffer
     // (fx) exists only when the whole mesh is resident and there is room (test tap cgks_debug_stage) or in the three-kernel
-    // pipeline (CGKS_PIPELINE=split, kept for A/B timing).
+    // pipeline (test-only A/B build, -DCGKS_AB_SPLIT_PIPELINE).
     const size_t left = (size_t)(end - p);
     const size_t sb = c->split ? slot_bytes(m.plane) : slot_bytes_pv(m.plane);
     long slots = (long)(left / sb);

@@ -152,7 +152,7 @@ def test_slab_pipeline_equals_resident():
     full, _ = parity.run_gpu(w, 2)
     n = 12 ** 3
     fixed = 3 * 80 * n * 8 + 5 * n * 8 + 37 * n * 8 + 4096
-    slot = 480 + (360 if os.environ.get("CGKS_PIPELINE") == "split" else 0)      # the three-kernel pipeline also holds face fluxes
+    slot = 480
     budget = fixed + 6 * slot * 144 * 8                  # 6 slots of reconstructed face values -> slab depth 4 -> 3 chunks
     s = binding.Solver(w["nodes"], binding.make_params(**w["params"], nonlinear=1), budget_bytes=budget)
     assert s.slab_depth() == 4
@@ -166,9 +166,12 @@ def test_slab_pipeline_equals_resident():
 @pytest.mark.parametrize("case", ["tgv_curv", "iso_sup", "ragged", "jump"])
 def test_sweep_pipeline_against_the_three_kernel_pipeline(case, monkeypatch):
     """The product path does flux + update in one sweep kernel per face direction (csrc/kernels_fused.cuh); the
-    three-kernel pipeline of rounds 1-2 (flux -> face-flux buffer -> update, CGKS_PIPELINE=split) is kept for A/B timing.
+    three-kernel pipeline of rounds 1-2 (flux -> face-flux buffer -> update) lives on in the TEST-ONLY build libcgks_ab.so
+    (build.build_ab(), -DCGKS_AB_SPLIT_PIPELINE), loaded here in place of the product library for the second run.
     They order the sums of Eq. 8-9 differently (direction by direction and Gauss-point quads against face by face), so
     they agree to round-off, not bit for bit; both match the oracle at 1e-10 per step."""
+    from paper_2508_08965_b200 import binding, build
+    ab_path = build.build_ab()
     if case == "ragged":
         nodes = inputs.cartesian_nodes((13, 9, 7), 0.0, 2.0 * np.pi); nodes[1] *= 0.8; nodes[2] *= 1.3
         w = dict(nodes=nodes, Q=inputs.taylor_green(nodes), G=None, D=None, params=inputs.tgv_params(Re=100.0), nonlinear=1, cfl=0.5)
@@ -177,11 +180,13 @@ def test_sweep_pipeline_against_the_three_kernel_pipeline(case, monkeypatch):
     else:
         w = parity.build_case(case, 12, 1, 2.0 if case == "iso_sup" else None)
     orc, dts = parity.run_oracle(w, 2)
-    monkeypatch.delenv("CGKS_PIPELINE", raising=False)
+    assert b"TEST BUILD" not in binding.lib().cgks_version()
     sweep, _ = parity.run_gpu(w, 2, dts=dts)
-    monkeypatch.setenv("CGKS_PIPELINE", "split")
+    monkeypatch.setattr(binding, "LIB_PATH", ab_path); monkeypatch.setattr(binding, "_lib", None)
+    assert b"TEST BUILD" in binding.lib().cgks_version()
     split, _ = parity.run_gpu(w, 2, dts=dts)
-    monkeypatch.delenv("CGKS_PIPELINE", raising=False)
+    monkeypatch.undo()                                   # back to the product library (the cached handle is restored with it)
+    assert b"TEST BUILD" not in binding.lib().cgks_version()
     e_ab = parity.field_errors(sweep, split, w["nodes"], w["Q"])
     e_sw = parity.field_errors(sweep, orc, w["nodes"], w["Q"])
     e_sp = parity.field_errors(split, orc, w["nodes"], w["Q"])
@@ -201,7 +206,7 @@ def test_sweep_lines_cut_into_segments():
     _check(w, 1, TOL_1)
     full, _ = parity.run_gpu(w, 2)
     n = shape[0] * shape[1] * shape[2]; plane = shape[0] * shape[1]
-    slot = 480 + (360 if os.environ.get("CGKS_PIPELINE") == "split" else 0)
+    slot = 480
     budget = 3 * 80 * n * 8 + 5 * n * 8 + 37 * n * 8 + 4096 + 30 * slot * plane * 8
     s = binding.Solver(w["nodes"], binding.make_params(**w["params"], nonlinear=1), budget_bytes=budget)
     assert 24 < s.slab_depth() < shape[2]          # two chunks, the first longer than the shortest segment
