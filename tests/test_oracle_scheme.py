@@ -183,6 +183,23 @@ def test_P6_table2_pattern():
     assert l1_nl < 2.0 * gold[(2, 10)][0]
 
 
+def test_P6c_table2_row_at_the_best_fit():
+    """Table 2's 10^3 row (L1 3.2325e-2, L2 1.2403e-2) is the one printed number that exercises the GENO blend.
+    The scan of DESIGN.md section 3.2 (oracle/readings_table.py --geno-scan) finds that reading G2 (B) with r = 2 reproduces it to
+    2 % at C = 3.5 (CFL 0.5); a wrong power in alpha, a missing square, IS^tau from the wrong derivative orders or a different
+    tanh map all move the row by 10 % or more (the scan's neighbours and negative controls), so 3 % pins the FORM of the path
+    function to the paper's number.  The default C = 5 (kept because only it leaves the 20^3 row identical to the linear one,
+    section 3.2) misses the row by -23 % / -18 %: pinned too, so that a change of the default or of the blend is noticed."""
+    from oracle import readings_table
+    p1, p2 = readings_table.TABLE2[10]
+    l1, l2 = readings_table.run(10, 1, C=3.5, cfl=0.5)
+    assert abs(l1 / p1 - 1.0) < 0.03 and abs(l2 / p2 - 1.0) < 0.03, (l1, l2)
+    l1, l2 = readings_table.run(10, 1, C=5.0, cfl=0.5)
+    assert abs(l1 / p1 - (1.0 - 0.231)) < 0.01 and abs(l2 / p2 - (1.0 - 0.177)) < 0.01, (l1, l2)
+    l1, l2 = readings_table.run(10, 1, C=4.0, cfl=0.5, g2=2)          # negative control: fourth-derivative part only
+    assert l1 / p1 < 0.80
+
+
 def test_P6b_nonlinear_equals_linear_at_20():
     """Short 20^3 run: nonlinear and linear results agree to ~1e-6 relative of the perturbation (Table 2 rows >= 20^3)."""
     a = run_sine(20, 0, tend=0.1)[3]; b = run_sine(20, 1, tend=0.1)[3]
